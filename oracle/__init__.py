@@ -1,0 +1,185 @@
+"""CPU oracle for the HEGET hot path -- TEST INFRASTRUCTURE, not product code.
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package.  It builds ``oracle/*.c`` with gcc
+into ``oracle/libheget_oracle.so`` and exposes the C entry points through ctypes with
+numpy arrays.  It imports nothing from the CUDA package and shares no code with it.
+
+Functions (all citations are PAPER.md lines, see the C sources):
+  amp(mom, nhel, g, gauge_idx=-1, extended=False)  one helicity amplitude (List 2)
+  amp2(momenta, g, extended=False)                 sum over helicities of |M|^2 (eq. 2)
+  gen_events(...)                                  Philox + RAMBO + boost + cuts + weight
+  xsec_reduce(amp2, weight, n)                     step 6 sums
+  philox4x32_10(ctr, key), uniforms(seed, event, slot), phase_space_volume(n, s)
+"""
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libheget_oracle.so")
+_SOURCES = ["heget_oracle.c", "heget_oracle_gen.c"]
+_DEPS = _SOURCES + ["amp_body.inc"]
+_lib = None
+
+# Couplings of DESIGN.md reading R2: alpha = 1/128, Q_u = 2/3, g = gal[0] = gal[1] = -e Q_u
+ALPHA = 1.0 / 128.0
+Q_U = 2.0 / 3.0
+G_DEFAULT = -Q_U * float(np.sqrt(4.0 * np.pi * ALPHA))
+
+
+def build(force=False):
+    """Compile the oracle with gcc (plain C99 + OpenMP, no FMA contraction)."""
+    srcs = [os.path.join(_HERE, s) for s in _SOURCES]
+    deps = [os.path.join(_HERE, s) for s in _DEPS]
+    if (not force and os.path.exists(_LIB_PATH)
+            and all(os.path.getmtime(_LIB_PATH) >= os.path.getmtime(d) for d in deps)):
+        return _LIB_PATH
+    cmd = ["gcc", "-std=gnu99", "-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC",
+           "-o", _LIB_PATH] + srcs + ["-lm"]
+    subprocess.run(cmd, check=True, cwd=_HERE)
+    return _LIB_PATH
+
+
+def _load():
+    global _lib
+    if _lib is not None:
+        return _lib
+    build()
+    lib = ctypes.CDLL(_LIB_PATH)
+    dp = ctypes.POINTER(ctypes.c_double)
+    ip = ctypes.POINTER(ctypes.c_int)
+    u32p = ctypes.POINTER(ctypes.c_uint32)
+    for name in ("heget_oracle_amp_d", "heget_oracle_amp_ld"):
+        f = getattr(lib, name)
+        f.argtypes = [dp, ctypes.c_int, ip, ctypes.c_double, ctypes.c_int, dp]
+        f.restype = None
+    for name in ("heget_oracle_amp2_d", "heget_oracle_amp2_ld"):
+        f = getattr(lib, name)
+        f.argtypes = [dp, ctypes.c_int, ctypes.c_int64, ctypes.c_double, dp]
+        f.restype = None
+    lib.heget_oracle_num_threads.restype = ctypes.c_int
+    lib.heget_oracle_philox4x32_10.argtypes = [u32p, u32p, u32p]
+    lib.heget_oracle_philox4x32_10.restype = None
+    lib.heget_oracle_uniforms.argtypes = [ctypes.c_uint64, ctypes.c_uint64, ctypes.c_uint32, dp]
+    lib.heget_oracle_uniforms.restype = None
+    lib.heget_oracle_phase_space_volume.argtypes = [ctypes.c_int, ctypes.c_double]
+    lib.heget_oracle_phase_space_volume.restype = ctypes.c_double
+    lib.heget_oracle_gen_events.argtypes = [
+        ctypes.c_uint64, ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_double,
+        ctypes.c_double, ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_double,
+        ctypes.c_uint64, ctypes.c_int64, dp, dp]
+    lib.heget_oracle_gen_events.restype = None
+    lib.heget_oracle_xsec_reduce.argtypes = [dp, dp, ctypes.c_int64, ctypes.c_int, dp]
+    lib.heget_oracle_xsec_reduce.restype = None
+    lib.heget_oracle_gamma.argtypes = [ctypes.c_int, dp]
+    lib.heget_oracle_gamma.restype = None
+    lib.heget_oracle_wavefunction.argtypes = [ctypes.c_int, dp, ctypes.c_int, ctypes.c_int, dp]
+    lib.heget_oracle_wavefunction.restype = None
+    _lib = lib
+    return lib
+
+
+def _dptr(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+def num_threads():
+    return int(_load().heget_oracle_num_threads())
+
+
+def amp(mom, nhel, g=G_DEFAULT, gauge_idx=-1, extended=False):
+    """ampsum (complex) for one event mom[n+2][4] and one helicity assignment nhel[n+2]."""
+    lib = _load()
+    mom = np.ascontiguousarray(mom, dtype=np.float64)
+    n = mom.shape[0] - 2
+    assert mom.shape == (n + 2, 4) and 1 <= n <= 8
+    nh = np.ascontiguousarray(nhel, dtype=np.int32)
+    assert nh.shape == (n + 2,) and np.all(np.abs(nh) == 1)
+    out = np.zeros(2, dtype=np.float64)
+    f = lib.heget_oracle_amp_ld if extended else lib.heget_oracle_amp_d
+    f(_dptr(mom), n, nh.ctypes.data_as(ctypes.POINTER(ctypes.c_int)), float(g), int(gauge_idx),
+      _dptr(out))
+    return complex(out[0], out[1])
+
+
+def amp2(momenta, g=G_DEFAULT, extended=False):
+    """Sum over all 4*2^n helicities of |M|^2 for momenta[N][n+2][4] -> [N]."""
+    lib = _load()
+    momenta = np.ascontiguousarray(momenta, dtype=np.float64)
+    assert momenta.ndim == 3 and momenta.shape[2] == 4
+    N, n = momenta.shape[0], momenta.shape[1] - 2
+    assert 1 <= n <= 8
+    out = np.zeros(N, dtype=np.float64)
+    if N == 0:
+        return out
+    f = lib.heget_oracle_amp2_ld if extended else lib.heget_oracle_amp2_d
+    f(_dptr(momenta), n, N, float(g), _dptr(out))
+    return out
+
+
+def gamma(mu):
+    """gamma^mu as a complex 4x4 numpy array (chiral representation)."""
+    out = np.zeros(32, dtype=np.float64)
+    _load().heget_oracle_gamma(int(mu), _dptr(out))
+    return (out[0::2] + 1j * out[1::2]).reshape(4, 4)
+
+
+def wavefunction(which, p, nhel, ns):
+    """which in {'i','o','v'}: ixxxx0 / oxxxx0 / vxxxx0 first four components."""
+    p = np.ascontiguousarray(p, dtype=np.float64)
+    out = np.zeros(8, dtype=np.float64)
+    _load().heget_oracle_wavefunction({"i": 0, "o": 1, "v": 2}[which], _dptr(p), int(nhel),
+                                      int(ns), _dptr(out))
+    return out[0::2] + 1j * out[1::2]
+
+
+def philox4x32_10(ctr, key):
+    lib = _load()
+    c = np.ascontiguousarray(ctr, dtype=np.uint32)
+    k = np.ascontiguousarray(key, dtype=np.uint32)
+    o = np.zeros(4, dtype=np.uint32)
+    u32p = ctypes.POINTER(ctypes.c_uint32)
+    lib.heget_oracle_philox4x32_10(c.ctypes.data_as(u32p), k.ctypes.data_as(u32p),
+                                   o.ctypes.data_as(u32p))
+    return o
+
+
+def uniforms(seed, event, slot):
+    lib = _load()
+    u = np.zeros(4, dtype=np.float64)
+    lib.heget_oracle_uniforms(int(seed), int(event), int(slot), _dptr(u))
+    return u
+
+
+def phase_space_volume(n, s):
+    return float(_load().heget_oracle_phase_space_volume(int(n), float(s)))
+
+
+MODE_FIXED, MODE_LOGUNIFORM, MODE_TOYPDF = 0, 1, 2
+
+
+def gen_events(seed, n, N, mode=MODE_FIXED, a=1000.0, b=0.0, y_max=0.0, apply_cuts=False,
+               pt_cut=20.0, eta_cut=2.5, dr_cut=0.4, first_event=0):
+    """Returns (momenta[N][n+2][4], weight[N]); see heget_oracle_gen.c for the modes."""
+    lib = _load()
+    momenta = np.zeros((N, n + 2, 4), dtype=np.float64)
+    weight = np.zeros(N, dtype=np.float64)
+    if N > 0:
+        lib.heget_oracle_gen_events(int(seed), int(n), int(mode), float(a), float(b), float(y_max),
+                                    int(bool(apply_cuts)), float(pt_cut), float(eta_cut),
+                                    float(dr_cut), int(first_event), int(N), _dptr(momenta),
+                                    _dptr(weight))
+    return momenta, weight
+
+
+def xsec_reduce(amp2_values, weight, n):
+    lib = _load()
+    a = np.ascontiguousarray(amp2_values, dtype=np.float64)
+    w = np.ascontiguousarray(weight, dtype=np.float64)
+    assert a.shape == w.shape and a.ndim == 1
+    out = np.zeros(3, dtype=np.float64)
+    lib.heget_oracle_xsec_reduce(_dptr(a), _dptr(w), a.shape[0], int(n), _dptr(out))
+    return out
