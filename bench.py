@@ -1,0 +1,300 @@
+#!/usr/bin/env python
+"""bench.py -- events/s of the summed squared helicity amplitude of u ubar -> n gamma on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4gamma] [--precision fp64]
+                    [--impl ours|reference] [--no-sweep]
+
+A step is one pass of the hot path over one batch of the named synthetic workload:
+heget_amp2 (rows a1-a8 of DESIGN.md) followed by heget_xsec_reduce (a9-a10), inputs (momenta,
+weights) resident in HBM.  `e2e` is the same through heget_xsec_host with pinned HOST buffers
+(H2D and D2H copies inside the timed region).  One JSON line is printed by rank 0.
+"""
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "events/s of summed |M|^2 for u ubar->n gamma"
+UNIT = "events/s"
+
+
+def model_flops_per_event(n):
+    """Model C of DESIGN.md: permutation tree with prefix reuse, Weyl form, the 2*2^n non-zero
+    helicity assignments; 44 flop per internal node, 24 per leaf (FMA = 2)."""
+    internal = sum(math.factorial(n) // math.factorial(n - l) for l in range(1, n))
+    return 2 * 2 ** n * (44 * internal + 24 * math.factorial(n))
+
+
+def theoretical_peak(precision, sm_count, sm_max_mhz):
+    lanes = 128 if precision == "fp32" else 64       # FP32 / FP64 FMA lanes per SM on B200
+    return sm_count * lanes * 2 * sm_max_mhz * 1e6
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self._stop, self._t = index, [], threading.Event(), None
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True,
+                                     timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([x.strip() for x in out.split(",")])
+            except Exception:
+                pass
+            self._stop.wait(0.1)
+
+    def start(self):
+        self._t = threading.Thread(target=self._run, daemon=True)
+        self._t.start()
+
+    def stop(self):
+        self._stop.set()
+        if self._t:
+            self._t.join(timeout=6)
+        sm = sorted(float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit())
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [nm for i, nm in enumerate(names) if any(len(r) > 3 + i and r[3 + i] == "Active" for r in self.rows)]
+        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(self.rows)}
+
+
+def oracle_sample_events(cfg, seconds_budget=15.0):
+    """How many events of this config the oracle is timed on (bounded CPU work)."""
+    per_event_core_s = {2: 2e-6, 3: 2.5e-5, 4: 2.4e-4, 5: 3.3e-3, 6: 5e-2, 7: 0.8, 8: 13.0}[cfg["n"]] * 8
+    cores = os.cpu_count() or 1
+    want = int(seconds_budget * cores / per_event_core_s)
+    return max(min(want, cfg["oracle_events"], cfg["N"]), min(cores, 4))
+
+
+def time_oracle(cfg, n_events):
+    """The oracle as it stands (oracle<double>, OpenMP over its own events) on the host cores."""
+    import oracle
+    from paper_0908_4403_b200 import workloads
+    mom, _ = oracle.gen_events(cfg["seed"], cfg["n"], n_events, mode=cfg["mode"], a=cfg["a"], b=cfg["b"],
+                               y_max=cfg["y_max"], apply_cuts=cfg["apply_cuts"], pt_cut=workloads.PT_CUT,
+                               eta_cut=workloads.ETA_CUT, dr_cut=workloads.DR_CUT)
+    t0 = time.perf_counter()
+    oracle.amp2(mom)
+    dt = time.perf_counter() - t0
+    return n_events / dt, dt, oracle.num_threads()
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on the host cores, same config/metric/unit."""
+    from paper_0908_4403_b200 import workloads
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    cfg = workloads.CONFIGS[args.config]
+    n_ev = oracle_sample_events(cfg, seconds_budget=8.0)
+    for _ in range(args.warmup):
+        time_oracle(cfg, max(n_ev // 8, 1))
+    total, cores = 0.0, 1
+    for _ in range(args.steps):
+        _, dt, cores = time_oracle(cfg, n_ev)
+        total += dt
+    value = n_ev * args.steps / total
+    sample = "first %d of %d events of %s per step, oracle<double>, OpenMP" % (n_ev, cfg["N"], args.config)
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": args.config, "n_photons": cfg["n"], "events_per_step": n_ev},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def time_config(hg, torch, name, precision, steps, warmup, flush, first_event, n_local):
+    """Device-timed steps of amp2 + xsec_reduce on resident inputs.  Returns per-step ms (whole
+    step) and the amp2 kernel's own ms, both from CUDA events on the launching stream."""
+    from paper_0908_4403_b200 import FP32, FP64, workloads
+    cfg = workloads.CONFIGS[name]
+    prec = FP64 if precision == "fp64" else FP32
+    mom, w = hg.gen_events(cfg["seed"], cfg["n"], n_local, mode=cfg["mode"], a=cfg["a"], b=cfg["b"],
+                           y_max=cfg["y_max"], apply_cuts=cfg["apply_cuts"], first_event=first_event)
+    amp2 = torch.empty(n_local, dtype=torch.float64, device=hg.device)
+    out3 = torch.empty(3, dtype=torch.float64, device=hg.device)
+
+    def step(ev=None):
+        if ev:
+            ev[0].record()
+        hg.amp2(mom, prec, out=amp2)
+        if ev:
+            ev[1].record()
+        hg.xsec_reduce(amp2, w, cfg["n"], out3=out3)
+        if ev:
+            ev[2].record()
+
+    for _ in range(warmup):
+        step()
+    torch.cuda.synchronize()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(steps)]
+    return mom, w, out3, step, evs, flush
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="4gamma")
+    ap.add_argument("--precision", default="fp64", choices=["fp32", "fp64"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-sweep", action="store_true", help="skip the per-n / per-precision table")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    if args.impl == "reference":
+        run_reference(args)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_0908_4403_b200 import FP32, FP64, Heget, workloads
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    hg = Heget(local_rank, workloads.ALPHA, workloads.Q_U, workloads.PT_CUT, workloads.ETA_CUT, workloads.DR_CUT)
+    cfg = workloads.CONFIGS[args.config]
+    n = cfg["n"]
+    # weak scaling: every rank processes the full per-GPU batch of the config, on its own
+    # contiguous range of global event indices (no data-path collective; the three sums of
+    # the reduction are all-reduced once per step)
+    n_local = cfg["N"]
+    first_event = rank * n_local
+    flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device=hg.device)   # > 126 MB L2
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed_run(name, precision, steps, warmup):
+        c = workloads.CONFIGS[name]
+        nl = c["N"]
+        mom, w, out3, step, evs, _ = time_config(hg, torch, name, precision, steps, warmup, None, rank * nl, nl)
+        barrier()
+        for ev in evs:
+            flush_buf.zero_()                                  # L2 flush, outside the timed events
+            step(ev)
+            if world > 1:
+                dist.all_reduce(out3)
+        barrier()
+        step_ms = [e[0].elapsed_time(e[2]) for e in evs]
+        amp_ms = [e[0].elapsed_time(e[1]) for e in evs]
+        return sum(step_ms), sum(amp_ms) / len(amp_ms), min(amp_ms), out3.cpu().numpy(), nl
+
+    launches0 = hg.launch_count()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    total_ms, amp_ms, amp_ms_best, sums, nl = timed_run(args.config, args.precision, args.steps, args.warmup)
+    clocks = sampler.stop()
+    launches = hg.launch_count() - launches0 - 3 * args.warmup - 1   # minus warm-up steps and the generator
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device=hg.device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = t.item()
+    value = world * nl * args.steps / (total_ms * 1e-3)
+
+    # end to end through the host-buffer entry point (pinned host inputs, H2D + D2H inside)
+    mom_d, w_d = hg.gen_events(cfg["seed"], n, nl, mode=cfg["mode"], a=cfg["a"], b=cfg["b"], y_max=cfg["y_max"],
+                               apply_cuts=cfg["apply_cuts"], first_event=first_event)
+    mom_h = torch.empty(mom_d.shape, dtype=torch.float64).pin_memory()
+    w_h = torch.empty(w_d.shape, dtype=torch.float64).pin_memory()
+    mom_h.copy_(mom_d)
+    w_h.copy_(w_d)
+    out3_h = torch.empty(3, dtype=torch.float64).pin_memory()
+    prec = FP64 if args.precision == "fp64" else FP32
+    for _ in range(2):
+        hg.xsec_host(mom_h, w_h, prec, out3=out3_h)
+    barrier()
+    e2e_steps = max(1, min(args.steps, 5))
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        hg.xsec_host(mom_h, w_h, prec, out3=out3_h)
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device=hg.device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = t.item()
+    e2e_value = world * nl * e2e_steps / e2e_s
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # roofline of the dominant kernel (amp2): plain-ALU bound, model-C flops over its own time
+    peak_measured = hg.fma_peak(prec)
+    sm_max = clocks["sm_max_mhz"] or 1965.0
+    peak_theory = theoretical_peak(args.precision, torch.cuda.get_device_properties(local_rank).multi_processor_count, sm_max)
+    achieved = model_flops_per_event(n) * nl / (amp_ms * 1e-3)
+    roofline = {"bound": "alu", "achieved": achieved / 1e12, "peak": peak_measured / 1e12, "unit": "TFLOP/s",
+                "frac": achieved / peak_measured, "traffic": None, "kernel": "amp2_kernel<%d,%s>" % (n, "double" if prec == FP64 else "float"),
+                "kernel_ms": amp_ms, "kernel_ms_best": amp_ms_best, "peak_theoretical": peak_theory / 1e12,
+                "frac_of_theoretical": achieved / peak_theory,
+                "flops_model": "C: DFS tree, Weyl form, non-zero helicities; 44/node, 24/leaf (kernel also uses the parity relation, so its executed flops are about half of C)",
+                "peak_source": "heget_fma_peak microbenchmark on this GPU (MEASURED_PEAKS.json has no non-tensor figure)"}
+
+    result = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+              "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+              "scaling": "weak", "vs_baseline": None, "dtype": "f64" if prec == FP64 else "f32",
+              "data": "synthetic",
+              "config": {"workload": args.config, "n_photons": n, "events_per_gpu": nl,
+                         "generation": "device Philox4x32-10 + RAMBO, seed %d" % cfg["seed"],
+                         "l2": "256 MiB buffer written between timed steps (L2 flush)"},
+              "clocks": clocks,
+              "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(mom_h.numel() * 8 + w_h.numel() * 8),
+                      "d2h_bytes_per_step": 24, "steps": e2e_steps},
+              "gpu_launches": int(launches),
+              "roofline": roofline,
+              "xsec": {"sum_wA": float(sums[0]), "sum_wA2": float(sums[1]), "n_pass": float(sums[2])}}
+
+    if not args.no_cpu_baseline:
+        n_ev = oracle_sample_events(cfg)
+        v, dt, cores = time_oracle(cfg, n_ev)
+        result["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                  "sample": "first %d of %d events of %s, oracle<double>, %.1f s" % (n_ev, cfg["N"], args.config, dt)}
+
+    if not args.no_sweep and world == 1:
+        table = []
+        for name in workloads.ORDER:
+            for precision in ("fp32", "fp64"):
+                _, a_ms, a_best, _, nn = timed_run(name, precision, 3, 3)
+                nph = workloads.CONFIGS[name]["n"]
+                pk = peak_measured if precision == args.precision else hg.fma_peak(FP64 if precision == "fp64" else FP32)
+                ach = model_flops_per_event(nph) * nn / (a_ms * 1e-3)
+                table.append({"workload": name, "n": nph, "precision": precision, "events": nn,
+                              "amp2_ms": a_ms, "events_per_s": nn / (a_ms * 1e-3),
+                              "model_tflops": ach / 1e12, "frac_of_measured_peak": ach / pk})
+        result["per_config"] = table
+
+    print(json.dumps(result))
+    hg.close()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,132 @@
+/* heget.h -- C ABI of libheget.so: B200 (sm_100a) evaluation of the summed squared
+ * helicity amplitude of u ubar -> n gamma, n = 2..8 (arXiv 0908.4403, "HEGET").
+ *
+ * Citations are PAPER.md line numbers of the paper text this library was written from.
+ *
+ * Conventions common to all calls
+ *  - every function returns 0 (HEGET_OK) or a negative HEGET_E* code; nothing aborts and
+ *    nothing throws across this boundary; heget_strerror() gives the text, and for
+ *    HEGET_ECUDA heget_last_cuda_error() gives the CUDA runtime's message;
+ *  - pointers marked [dev] are device pointers on the context's device, owned by the
+ *    caller (e.g. a torch tensor's data_ptr()); pointers marked [host] are host pointers
+ *    (pinned or pageable).  The library allocates nothing per call for the [dev] entry
+ *    points; the *_host entry points use staging buffers owned by the context;
+ *  - [dev] calls are asynchronous on `stream` (a cudaStream_t passed as void*, NULL = the
+ *    legacy default stream) and do not synchronise the host; *_host calls return after
+ *    the result is in the host buffer;
+ *  - momenta layout: double[N][n+2][4], four-vectors (E,px,py,pz) (PAPER.md:474-477,
+ *    553-554), particle order u, ubar, gamma_1..gamma_n (p1..p5 of List 2);
+ *    the base pointer must be 16-byte aligned.
+ *  - preconditions (documented, not checked on the hot path; PAPER.md:203-205 makes the
+ *    same assumptions by choosing ixxxx1 / oxxxx2 / branch-free vxxxx0):
+ *    p1 = (E1,0,0,+E1), p2 = (E2,0,0,-E2), photons massless to rounding with pT > 0.
+ */
+#ifndef HEGET_H
+#define HEGET_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct heget_ctx heget_ctx; /* opaque; owned by the library */
+
+enum { HEGET_FP32 = 0, HEGET_FP64 = 1 };
+
+enum {
+    HEGET_OK = 0,
+    HEGET_EINVAL = -1, /* n outside [2,8], N < 0, null pointer, bad precision/mode */
+    HEGET_ECUDA = -2,  /* a CUDA runtime call or launch failed */
+    HEGET_ENOMEM = -3  /* host or device allocation failed */
+};
+
+/* Event-generation modes of heget_gen_events ("input recipe"). */
+enum {
+    HEGET_GEN_FIXED = 0,      /* sqrt_s_hat = a, y = 0 */
+    HEGET_GEN_LOGUNIFORM = 1, /* sqrt_s_hat = a (b/a)^u log-uniform in [a,b], y uniform in [-y_max,y_max] */
+    HEGET_GEN_TOYPDF = 2      /* pp at sqrt(s) = a with f(x) = x^-0.5 (1-x)^3 for both partons */
+};
+
+typedef struct heget_gen_cfg {
+    int mode;       /* HEGET_GEN_* */
+    int apply_cuts; /* 0: weight never zeroed; 1: eq. (9) cuts from the context */
+    double a;       /* see mode */
+    double b;       /* see mode */
+    double y_max;   /* HEGET_GEN_LOGUNIFORM only */
+} heget_gen_cfg;
+
+/* Create a context on CUDA device `device`.
+ *   alpha, q_charge : fine-structure constant and quark charge; the FFV coupling is
+ *                     gal[0] = gal[1] = -e Q_q, e = sqrt(4 pi alpha) (eq. 26)
+ *   pt_cut, eta_cut, dr_cut : final-state cuts of eq. (9)
+ * *out is written on success only and must be released with heget_destroy. */
+int heget_init(int device, double alpha, double q_charge, double pt_cut, double eta_cut,
+               double dr_cut, heget_ctx** out);
+void heget_destroy(heget_ctx* ctx);
+const char* heget_strerror(int code);
+const char* heget_last_cuda_error(const heget_ctx* ctx);
+
+/* Phase space generation from random numbers, step 4 of PAPER.md:116-122 ("generates a
+ * phase space point and computes a Jacobian") with device-side Philox4x32-10
+ * and RAMBO (neither is named by the paper; BASELINE.json fixes them, R6/R7).
+ * heget_rambo is the north-star form: fixed sqrt_s_hat, partonic rest frame, u along +z,
+ * ubar along -z, no cuts.  Event e uses Philox counter (e, slot) with key `seed`.
+ *   momenta [dev] double[N][n+2][4], written. */
+int heget_rambo(heget_ctx* ctx, uint64_t seed, int n, double sqrt_s_hat, int64_t N,
+                double* momenta, void* stream);
+
+/* General form: per-event sqrt_s_hat and boost rapidity y according to cfg, cuts of eq. (9)
+ * evaluated in the boosted frame, and the event weight
+ *   w = [cuts] * Phi_n(s_hat) / (2 s_hat) * (TOYPDF: Jacobian * 2 f(x1) f(x2))
+ * (eqs. 1-4).  Global event index = first_event + local index, so any
+ * contiguous shard of a run reproduces the same events (multi-GPU: shard by index range).
+ *   momenta [dev] double[N][n+2][4], weight [dev] double[N]; both written. */
+int heget_gen_events(heget_ctx* ctx, uint64_t seed, int n, const heget_gen_cfg* cfg,
+                     uint64_t first_event, int64_t N, double* momenta, double* weight,
+                     void* stream);
+
+/* The hot path.  For each event: external wavefunctions (ixxxx1, oxxxx2, vxxxx0;
+ * PAPER.md:435-439), the fvixx0 chain through the propagators (p1 - K_l)/t_l of eqs. (7),(8)
+ * over all n! photon orderings of eq. (6), walked
+ * as a depth-first permutation tree with every prefix computed once, closed by iovxxx
+ * (PAPER.md:592-620), squared and summed over all 4*2^n helicities:
+ *   out_amp2[e] = sum_{sigma1,sigma2,lambda_1..lambda_n} |M|^2   (the sum in eq. 2,
+ *   PAPER.md:37, WITHOUT 1/(2 s_hat), spin/colour average and 1/n!).
+ * precision selects the arithmetic of the tree walk (separate fp32 and fp64 kernels);
+ * input and output buffers are fp64 in both cases (the fp32 kernel rescales each event to
+ * unit s_hat internally because |M|^2 ~ s_hat^(2-n) leaves the fp32 range).
+ *   momenta [dev] const double[N][n+2][4]; out_amp2 [dev] double[N], written. */
+int heget_amp2(heget_ctx* ctx, const double* momenta, int n, int precision, double* out_amp2,
+               int64_t N, void* stream);
+
+/* Step 6 of PAPER.md:141 on the device: with x_e = weight[e] * amp2[e] * (1/4)(1/9)(1/n!)
+ * (helicity average, colour factor and identical-photon factor of eq. 2, PAPER.md:37;
+ * DESIGN.md R1 for the colour factor),
+ *   out3 = { sum_e x_e, sum_e x_e^2, #(weight[e] != 0) }   accumulated in fp64.
+ * The result is deterministic (fixed reduction tree, no floating-point atomics).
+ *   amp2, weight [dev] const double[N]; out3 [dev] double[3], written. */
+int heget_xsec_reduce(heget_ctx* ctx, const double* amp2, const double* weight, int n, int64_t N,
+                      double* out3, void* stream);
+
+/* End-to-end form of the same path with host buffers: copies momenta and weight to the
+ * device, runs heget_amp2 and heget_xsec_reduce, copies out_amp2 (if non-NULL) and out3
+ * back, and returns when they are in host memory.
+ *   momenta [host] const double[N][n+2][4]; weight [host] const double[N];
+ *   out_amp2 [host] double[N] or NULL; out3 [host] double[3]. */
+int heget_xsec_host(heget_ctx* ctx, const double* momenta, const double* weight, int n,
+                    int precision, int64_t N, double* out_amp2, double* out3);
+
+/* Peak-rate microbenchmark used for the roofline denominator: launches a kernel of
+ * independent FMA chains (precision = HEGET_FP32 / HEGET_FP64) filling every SM and
+ * writes the achieved FLOP/s (FMA = 2) to *flops_per_s [host].  Synchronises. */
+int heget_fma_peak(heget_ctx* ctx, int precision, double* flops_per_s);
+
+/* Number of kernel launches this context has issued (all entry points), for bench.py's
+ * gpu_launches count. */
+int64_t heget_launch_count(const heget_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HEGET_H */

@@ -1,0 +1,188 @@
+// amp2.cu -- heget_amp2: summed squared helicity amplitude of u ubar -> n gamma (product code).
+//
+// Mapping: one lane per photon-helicity configuration (2^N lanes per event), 256-thread CTAs
+// holding 256/2^N events.  All lanes of a CTA walk the SAME permutation tree in lockstep
+// (no divergence); they differ only in which helicity entry of the per-photon E table they
+// read.  Per event the CTA first builds, in shared memory,
+//   - the E table (vxxxx0 for both helicities of every photon) and
+//   - the subset table P[S] = -g/t_S * (p1 - K_S)-slash block for every photon subset S,
+// then every lane runs the depth-first walk of eq. (6)'s n! orderings: each
+// ordered prefix (tree node) is one fvixx0 computed once, each leaf one
+// iovxxx accumulated into ampsum (List 2).
+// Only sigma_1 = +1, sigma_2 = -1 is evaluated: sigma_1 = sigma_2 vanishes identically and
+// |M(-sigma,-lambda)| = |M(sigma,lambda)|, so the helicity sum is twice the sum over lambda.
+#include "amp2_tables.cuh"
+#include "heget_internal.cuh"
+
+namespace {
+
+template <typename T>
+struct Spinor {
+    T r0, i0, r1, i1;  // two complex components
+};
+
+// fvixx0 in Weyl form: psi' = P_S * (E_i * psi).
+template <typename T>
+__device__ __forceinline__ Spinor<T> fvixx0_weyl(const PEntry<T>& P, const EEntry<T>& E, const Spinor<T>& f)
+{
+    // w = E f,  E = [[-s, -B], [A, s]]
+    const T w0r = -E.s * f.r0 - (E.br * f.r1 - E.bi * f.i1);
+    const T w0i = -E.s * f.i0 - (E.br * f.i1 + E.bi * f.r1);
+    const T w1r = E.s * f.r1 + (E.ar * f.r0 - E.ai * f.i0);
+    const T w1i = E.s * f.i1 + (E.ar * f.i0 + E.ai * f.r0);
+    // psi' = P w,  P = [[pp, px - i py], [px + i py, pm]]
+    Spinor<T> o;
+    o.r0 = P.pp * w0r + (P.px * w1r + P.py * w1i);
+    o.i0 = P.pp * w0i + (P.px * w1i - P.py * w1r);
+    o.r1 = P.pm * w1r + (P.px * w0r - P.py * w0i);
+    o.i1 = P.pm * w1i + (P.px * w0i + P.py * w0r);
+    return o;
+}
+
+// iovxxx in Weyl form: vbar (oxxxx2) has the single component 1 of the (0,1)
+// pair, so amp = row 1 of E_j times psi = A psi0 + s psi1 (constant factors applied at the end).
+template <typename T>
+__device__ __forceinline__ void iovxxx_weyl(const EEntry<T>& E, const Spinor<T>& f, T& ar, T& ai)
+{
+    ar += E.s * f.r1 + (E.ar * f.r0 - E.ai * f.i0);
+    ai += E.s * f.i1 + (E.ar * f.i0 + E.ai * f.r0);
+}
+
+// Depth-first walk.  `used` = set of photons already attached (uniform over the CTA).
+template <int N, int DEPTH, typename T>
+struct Walk {
+    static __device__ __forceinline__ void run(const PEntry<T>* __restrict__ P, const EEntry<T>* __restrict__ E,
+                                               unsigned hel, unsigned used, const Spinor<T>& f, T& ar, T& ai)
+    {
+        unsigned avail = ((1u << N) - 1u) & ~used;
+        if constexpr (DEPTH == N - 1) {
+            const int j = __ffs(avail) - 1;
+            iovxxx_weyl(E[2 * j + ((hel >> j) & 1u)], f, ar, ai);
+        } else {
+            while (avail) {
+                const int i = __ffs(avail) - 1;
+                avail &= avail - 1u;
+                const unsigned S = used | (1u << i);
+                const Spinor<T> fn = fvixx0_weyl(P[S], E[2 * i + ((hel >> i) & 1u)], f);
+                Walk<N, DEPTH + 1, T>::run(P, E, hel, S, fn, ar, ai);
+            }
+        }
+    }
+};
+
+template <int N>
+struct Geometry {
+    static constexpr int L = 1 << N;                       // lanes (helicity configurations) per event
+    static constexpr int THREADS = (L > 256) ? L : 256;
+    static constexpr int EPB = THREADS / L;                // events per CTA
+};
+
+template <int N, typename T>
+__global__ void __launch_bounds__(Geometry<N>::THREADS)
+amp2_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_t n_events, double g)
+{
+    using G = Geometry<N>;
+    constexpr int MOM = 4 * (N + 2);
+    __shared__ __align__(16) double s_mom[G::EPB * MOM];
+    __shared__ PEntry<T> s_P[G::EPB * G::L];
+    __shared__ EEntry<T> s_E[G::EPB * 2 * N];
+    __shared__ double s_red[G::THREADS / 32];
+
+    const int tid = threadIdx.x;
+    const int ev_local = tid / G::L;
+    const unsigned hel = tid % G::L;
+    const int64_t ev0 = (int64_t)blockIdx.x * G::EPB;
+
+    // a1: coalesced load of the CTA's momenta (events past the end re-read the last event)
+    {
+        const double2* src = reinterpret_cast<const double2*>(momenta);
+        double2* dst = reinterpret_cast<double2*>(s_mom);
+        for (int idx = tid; idx < G::EPB * MOM / 2; idx += G::THREADS) {
+            int64_t e = ev0 + idx / (MOM / 2);
+            if (e >= n_events) e = n_events - 1;
+            dst[idx] = src[e * (MOM / 2) + idx % (MOM / 2)];
+        }
+    }
+    __syncthreads();
+
+    const double* mom = s_mom + ev_local * MOM;
+    const double shat = 4.0 * mom[0] * mom[4];  // (p1+p2)^2 for p1 || +z, p2 || -z
+    const double scale = (sizeof(T) == 4) ? sqrt(shat) : 1.0;
+    // a4: vxxxx0 for both helicities of photon `hel` (lanes 0..N-1 of each event)
+    if (hel < (unsigned)N)
+        make_photon_entries<T>(mom + 4 * (2 + hel), &s_E[(ev_local * N + hel) * 2 + 1],
+                               &s_E[(ev_local * N + hel) * 2 + 0]);
+    // a5: subset kinematics, one subset per lane
+    if (hel >= 1u && hel <= (unsigned)(G::L - 2))
+        make_subset_entry<N, T>(mom, hel, g, scale, &s_P[ev_local * G::L + hel]);
+    __syncthreads();
+
+    // a2, a6, a7: psi_0 = u(p1,+)/sqrt(2E1) = (1,0); walk the permutation tree
+    T ar = 0, ai = 0;
+    const Spinor<T> f0 = {(T)1, (T)0, (T)0, (T)0};
+    Walk<N, 0, T>::run(s_P + ev_local * G::L, s_E + ev_local * 2 * N, hel, 0u, f0, ar, ai);
+
+    // a8: |ampsum|^2 summed over the event's 2^N lanes
+    double m2 = (double)ar * (double)ar + (double)ai * (double)ai;
+    constexpr int WL = (G::L < 32) ? G::L : 32;
+#pragma unroll
+    for (int off = WL / 2; off > 0; off >>= 1) m2 += __shfl_xor_sync(0xffffffffu, m2, off);
+    if constexpr (G::L > 32) {
+        if ((tid & 31) == 0) s_red[tid >> 5] = m2;
+        __syncthreads();
+        if (hel == 0) {
+            m2 = 0.0;
+#pragma unroll
+            for (int w = 0; w < G::L / 32; ++w) m2 += s_red[ev_local * (G::L / 32) + w];
+        }
+    }
+    if (hel == 0 && ev0 + ev_local < n_events) {
+        // constants: 2 (parity) * g^2 (closing vertex) * 2E1*2E2 = s_hat (spinor norms) * 2^-N
+        // (the sqrt(2) of every polarisation vector); fp32 worked in units of sqrt(s_hat)
+        double f = 2.0 * g * g * shat;
+#pragma unroll
+        for (int i = 0; i < N; ++i) f *= 0.5;
+        if (sizeof(T) == 4) {
+            const double inv = 1.0 / shat;
+#pragma unroll
+            for (int i = 0; i < N - 1; ++i) f *= inv;
+        }
+        out[ev0 + ev_local] = f * m2;
+    }
+}
+
+template <int N, typename T>
+cudaError_t launch_one(const double* momenta, double* out, int64_t n_events, double g, cudaStream_t stream)
+{
+    using G = Geometry<N>;
+    const int64_t blocks = (n_events + G::EPB - 1) / G::EPB;
+    amp2_kernel<N, T><<<(unsigned)blocks, G::THREADS, 0, stream>>>(momenta, out, n_events, g);
+    return cudaGetLastError();
+}
+
+template <typename T>
+cudaError_t launch_n(int n, const double* momenta, double* out, int64_t n_events, double g, cudaStream_t stream)
+{
+    switch (n) {
+        case 2: return launch_one<2, T>(momenta, out, n_events, g, stream);
+        case 3: return launch_one<3, T>(momenta, out, n_events, g, stream);
+        case 4: return launch_one<4, T>(momenta, out, n_events, g, stream);
+        case 5: return launch_one<5, T>(momenta, out, n_events, g, stream);
+        case 6: return launch_one<6, T>(momenta, out, n_events, g, stream);
+        case 7: return launch_one<7, T>(momenta, out, n_events, g, stream);
+        case 8: return launch_one<8, T>(momenta, out, n_events, g, stream);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+}  // namespace
+
+cudaError_t heget_launch_amp2(const heget_ctx* ctx, const double* momenta, int n, int precision,
+                              double* out_amp2, int64_t N, cudaStream_t stream, int* launches)
+{
+    *launches = 0;
+    if (N == 0) return cudaSuccess;
+    *launches = 1;
+    if (precision == HEGET_FP32) return launch_n<float>(n, momenta, out_amp2, N, ctx->g, stream);
+    return launch_n<double>(n, momenta, out_amp2, N, ctx->g, stream);
+}

@@ -1,0 +1,209 @@
+// api.cu -- the extern "C" boundary of libheget.so (include/heget.h).  Argument checking,
+// context bookkeeping and launches only; all arithmetic is in the kernels.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "heget_internal.cuh"
+
+namespace {
+
+int fail_cuda(heget_ctx* ctx, cudaError_t err)
+{
+    if (ctx) snprintf(ctx->cuda_msg, sizeof(ctx->cuda_msg), "%s: %s", cudaGetErrorName(err), cudaGetErrorString(err));
+    return HEGET_ECUDA;
+}
+
+struct DeviceGuard {
+    int prev = -1;
+    bool ok;
+    explicit DeviceGuard(int dev)
+    {
+        ok = cudaGetDevice(&prev) == cudaSuccess && (prev == dev || cudaSetDevice(dev) == cudaSuccess);
+        if (prev == dev) prev = -1;
+    }
+    ~DeviceGuard()
+    {
+        if (prev >= 0) cudaSetDevice(prev);
+    }
+};
+
+void free_staging(heget_ctx* ctx)
+{
+    cudaFree(ctx->d_stage_mom);
+    cudaFree(ctx->d_stage_w);
+    cudaFree(ctx->d_stage_amp2);
+    ctx->d_stage_mom = ctx->d_stage_w = ctx->d_stage_amp2 = nullptr;
+    ctx->stage_events = ctx->stage_n_events = 0;
+}
+
+}  // namespace
+
+extern "C" {
+
+int heget_init(int device, double alpha, double q_charge, double pt_cut, double eta_cut, double dr_cut,
+               heget_ctx** out)
+{
+    if (!out || !(alpha > 0.0) || device < 0) return HEGET_EINVAL;
+    int count = 0;
+    if (cudaGetDeviceCount(&count) != cudaSuccess || device >= count) return HEGET_ECUDA;
+    DeviceGuard guard(device);
+    if (!guard.ok) return HEGET_ECUDA;
+    heget_ctx* ctx = new (std::nothrow) heget_ctx();
+    if (!ctx) return HEGET_ENOMEM;
+    memset(ctx, 0, sizeof(*ctx));
+    ctx->device = device;
+    ctx->alpha = alpha;
+    ctx->q_charge = q_charge;
+    ctx->g = -q_charge * sqrt(4.0 * 3.14159265358979323846 * alpha);  // eq. (26)
+    ctx->pt_cut = pt_cut;
+    ctx->eta_cut = eta_cut;
+    ctx->dr_cut = dr_cut;
+    cudaDeviceProp prop;
+    cudaError_t err = cudaGetDeviceProperties(&prop, device);
+    if (err == cudaSuccess) {
+        ctx->sm_count = prop.multiProcessorCount;
+        err = cudaMalloc(&ctx->d_partials, sizeof(double) * 3 * kReduceBlocks);
+    }
+    if (err == cudaSuccess) err = cudaMalloc(&ctx->d_stage_out3, sizeof(double) * 3);
+    if (err == cudaSuccess) err = cudaStreamCreateWithFlags(&ctx->host_stream, cudaStreamNonBlocking);
+    if (err != cudaSuccess) {
+        cudaFree(ctx->d_partials);
+        cudaFree(ctx->d_stage_out3);
+        delete ctx;
+        return HEGET_ECUDA;
+    }
+    *out = ctx;
+    return HEGET_OK;
+}
+
+void heget_destroy(heget_ctx* ctx)
+{
+    if (!ctx) return;
+    DeviceGuard guard(ctx->device);
+    free_staging(ctx);
+    cudaFree(ctx->d_partials);
+    cudaFree(ctx->d_stage_out3);
+    if (ctx->host_stream) cudaStreamDestroy(ctx->host_stream);
+    delete ctx;
+}
+
+const char* heget_strerror(int code)
+{
+    switch (code) {
+        case HEGET_OK: return "success";
+        case HEGET_EINVAL: return "invalid argument (n outside [2,8], N < 0, null pointer, bad precision or mode)";
+        case HEGET_ECUDA: return "CUDA runtime error (see heget_last_cuda_error)";
+        case HEGET_ENOMEM: return "allocation failed";
+        default: return "unknown heget error code";
+    }
+}
+
+const char* heget_last_cuda_error(const heget_ctx* ctx) { return ctx ? ctx->cuda_msg : ""; }
+
+int64_t heget_launch_count(const heget_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int heget_gen_events(heget_ctx* ctx, uint64_t seed, int n, const heget_gen_cfg* cfg, uint64_t first_event,
+                     int64_t N, double* momenta, double* weight, void* stream)
+{
+    if (!ctx || !cfg || n < 2 || n > 8 || N < 0 || (N > 0 && !momenta)) return HEGET_EINVAL;
+    if (cfg->mode < HEGET_GEN_FIXED || cfg->mode > HEGET_GEN_TOYPDF || !(cfg->a > 0.0)) return HEGET_EINVAL;
+    if (cfg->mode == HEGET_GEN_LOGUNIFORM && !(cfg->b >= cfg->a)) return HEGET_EINVAL;
+    DeviceGuard guard(ctx->device);
+    if (!guard.ok) return fail_cuda(ctx, cudaGetLastError());
+    int launches = 0;
+    cudaError_t err = heget_launch_gen(ctx, seed, n, cfg, first_event, N, momenta, weight, (cudaStream_t)stream, &launches);
+    ctx->launches += launches;
+    return err == cudaSuccess ? HEGET_OK : fail_cuda(ctx, err);
+}
+
+int heget_rambo(heget_ctx* ctx, uint64_t seed, int n, double sqrt_s_hat, int64_t N, double* momenta, void* stream)
+{
+    heget_gen_cfg cfg;
+    cfg.mode = HEGET_GEN_FIXED;
+    cfg.apply_cuts = 0;
+    cfg.a = sqrt_s_hat;
+    cfg.b = 0.0;
+    cfg.y_max = 0.0;
+    return heget_gen_events(ctx, seed, n, &cfg, 0, N, momenta, nullptr, stream);
+}
+
+int heget_amp2(heget_ctx* ctx, const double* momenta, int n, int precision, double* out_amp2, int64_t N, void* stream)
+{
+    if (!ctx || n < 2 || n > 8 || N < 0 || (N > 0 && (!momenta || !out_amp2))) return HEGET_EINVAL;
+    if (precision != HEGET_FP32 && precision != HEGET_FP64) return HEGET_EINVAL;
+    if ((reinterpret_cast<uintptr_t>(momenta) & 15u) != 0) return HEGET_EINVAL;
+    DeviceGuard guard(ctx->device);
+    if (!guard.ok) return fail_cuda(ctx, cudaGetLastError());
+    int launches = 0;
+    cudaError_t err = heget_launch_amp2(ctx, momenta, n, precision, out_amp2, N, (cudaStream_t)stream, &launches);
+    ctx->launches += launches;
+    return err == cudaSuccess ? HEGET_OK : fail_cuda(ctx, err);
+}
+
+int heget_xsec_reduce(heget_ctx* ctx, const double* amp2, const double* weight, int n, int64_t N, double* out3,
+                      void* stream)
+{
+    if (!ctx || n < 2 || n > 8 || N < 0 || !out3 || (N > 0 && (!amp2 || !weight))) return HEGET_EINVAL;
+    DeviceGuard guard(ctx->device);
+    if (!guard.ok) return fail_cuda(ctx, cudaGetLastError());
+    int launches = 0;
+    cudaError_t err = heget_launch_reduce(ctx, amp2, weight, n, N, out3, (cudaStream_t)stream, &launches);
+    ctx->launches += launches;
+    return err == cudaSuccess ? HEGET_OK : fail_cuda(ctx, err);
+}
+
+int heget_xsec_host(heget_ctx* ctx, const double* momenta, const double* weight, int n, int precision, int64_t N,
+                    double* out_amp2, double* out3)
+{
+    if (!ctx || n < 2 || n > 8 || N < 0 || !out3 || (N > 0 && (!momenta || !weight))) return HEGET_EINVAL;
+    if (precision != HEGET_FP32 && precision != HEGET_FP64) return HEGET_EINVAL;
+    DeviceGuard guard(ctx->device);
+    if (!guard.ok) return fail_cuda(ctx, cudaGetLastError());
+    const int64_t need = N * (n + 2);
+    cudaError_t err = cudaSuccess;
+    if (need > ctx->stage_events || N > ctx->stage_n_events) {
+        free_staging(ctx);
+        const int64_t cap_n = N > 0 ? N : 1;
+        err = cudaMalloc(&ctx->d_stage_mom, sizeof(double) * 4 * cap_n * 10);
+        if (err == cudaSuccess) err = cudaMalloc(&ctx->d_stage_w, sizeof(double) * cap_n);
+        if (err == cudaSuccess) err = cudaMalloc(&ctx->d_stage_amp2, sizeof(double) * cap_n);
+        if (err != cudaSuccess) {
+            free_staging(ctx);
+            snprintf(ctx->cuda_msg, sizeof(ctx->cuda_msg), "%s", cudaGetErrorString(err));
+            return HEGET_ENOMEM;
+        }
+        ctx->stage_events = cap_n * 10;
+        ctx->stage_n_events = cap_n;
+    }
+    cudaStream_t st = ctx->host_stream;
+    int launches = 0, l2 = 0;
+    if (N > 0) {
+        err = cudaMemcpyAsync(ctx->d_stage_mom, momenta, sizeof(double) * 4 * need, cudaMemcpyHostToDevice, st);
+        if (err == cudaSuccess)
+            err = cudaMemcpyAsync(ctx->d_stage_w, weight, sizeof(double) * N, cudaMemcpyHostToDevice, st);
+        if (err == cudaSuccess)
+            err = heget_launch_amp2(ctx, ctx->d_stage_mom, n, precision, ctx->d_stage_amp2, N, st, &launches);
+    }
+    if (err == cudaSuccess) err = heget_launch_reduce(ctx, ctx->d_stage_amp2, ctx->d_stage_w, n, N, ctx->d_stage_out3, st, &l2);
+    ctx->launches += launches + l2;
+    if (err == cudaSuccess && out_amp2 && N > 0)
+        err = cudaMemcpyAsync(out_amp2, ctx->d_stage_amp2, sizeof(double) * N, cudaMemcpyDeviceToHost, st);
+    if (err == cudaSuccess) err = cudaMemcpyAsync(out3, ctx->d_stage_out3, sizeof(double) * 3, cudaMemcpyDeviceToHost, st);
+    if (err == cudaSuccess) err = cudaStreamSynchronize(st);
+    return err == cudaSuccess ? HEGET_OK : fail_cuda(ctx, err);
+}
+
+int heget_fma_peak(heget_ctx* ctx, int precision, double* flops_per_s)
+{
+    if (!ctx || !flops_per_s || (precision != HEGET_FP32 && precision != HEGET_FP64)) return HEGET_EINVAL;
+    DeviceGuard guard(ctx->device);
+    if (!guard.ok) return fail_cuda(ctx, cudaGetLastError());
+    int launches = 0;
+    cudaError_t err = heget_run_fma_peak(ctx, precision, flops_per_s, &launches);
+    ctx->launches += launches;
+    return err == cudaSuccess ? HEGET_OK : fail_cuda(ctx, err);
+}
+
+}  // extern "C"

@@ -1,0 +1,170 @@
+// gen.cu -- heget_rambo / heget_gen_events: device-side Philox4x32-10 + RAMBO + boost + cuts +
+// weight, one thread per event (product code; step 4 of PAPER.md:116-122, cuts of eq. 9
+// PAPER.md:89-96, weight from eqs. 1-4).  The paper draws its random numbers
+// on the CPU and copies them over; here the counter-based generator runs
+// in the kernel, keyed by the global event index, so nothing crosses PCIe.
+#include "heget_internal.cuh"
+
+namespace {
+
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                              uint32_t k0, uint32_t k1, uint32_t out[4])
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        const uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// key = seed, counter = (event_lo, event_hi, slot, 0); u = (x + 0.5) 2^-32 in (0,1)
+__device__ __forceinline__ void uniforms4(uint64_t seed, uint64_t event, uint32_t slot, double u[4])
+{
+    uint32_t x[4];
+    philox4x32_10((uint32_t)event, (uint32_t)(event >> 32), slot, 0u, (uint32_t)seed, (uint32_t)(seed >> 32), x);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) u[i] = ((double)x[i] + 0.5) * (1.0 / 4294967296.0);
+}
+
+__device__ __forceinline__ double phase_space_volume(int n, double s)
+{
+    // Phi_n(s) = (2 pi)^(4-3n) (pi/2)^(n-1) s^(n-2) / ((n-1)! (n-2)!)   (integral of eq. 4)
+    const double pi = 3.14159265358979323846;
+    double v = 1.0 / (8.0 * pi);  // n = 2
+    for (int m = 3; m <= n; ++m) v *= s * (pi / 2.0) / ((2.0 * pi) * (2.0 * pi) * (2.0 * pi)) / ((double)(m - 1) * (double)(m - 2));
+    return v;
+}
+
+template <int N>
+__global__ void __launch_bounds__(128)
+gen_kernel(uint64_t seed, heget_gen_cfg cfg, double pt_cut, double eta_cut, double dr_cut,
+           uint64_t first_event, int64_t n_events, double* __restrict__ momenta, double* __restrict__ weight)
+{
+    const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n_events) return;
+    const uint64_t ev = first_event + (uint64_t)e;
+    const double pi = 3.14159265358979323846;
+
+    double u0[4];
+    uniforms4(seed, ev, 0u, u0);
+    double rs, y, extra = 1.0;
+    if (cfg.mode == HEGET_GEN_FIXED) {
+        rs = cfg.a;
+        y = 0.0;
+    } else if (cfg.mode == HEGET_GEN_LOGUNIFORM) {
+        rs = cfg.a * pow(cfg.b / cfg.a, u0[0]);
+        y = cfg.y_max * (2.0 * u0[1] - 1.0);
+    } else {
+        const double s = cfg.a * cfg.a;
+        const double tau_min = (N * pt_cut) * (N * pt_cut) / s;
+        const double ln_tau_min = log(tau_min);
+        const double ln_tau = (1.0 - u0[0]) * ln_tau_min;
+        const double tau = exp(ln_tau);
+        y = (2.0 * u0[1] - 1.0) * (-0.5 * ln_tau);
+        const double x1 = sqrt(tau) * exp(y), x2 = sqrt(tau) * exp(-y);
+        const double o1 = 1.0 - x1, o2 = 1.0 - x2;
+        const double f1 = o1 * o1 * o1 / sqrt(x1), f2 = o2 * o2 * o2 / sqrt(x2);
+        rs = sqrt(tau * s);
+        extra = tau * (-ln_tau_min) * (-ln_tau) * 2.0 * f1 * f2;
+    }
+
+    // RAMBO: isotropic massless q_i, then the conformal boost and rescale to total (rs, 0)
+    double q[N][4], Q[4] = {0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+        double u[4];
+        uniforms4(seed, ev, (uint32_t)(i + 1), u);
+        const double c = 2.0 * u[0] - 1.0;
+        const double s = sqrt(1.0 - c * c);
+        double sf, cf;
+        sincos(2.0 * pi * u[1], &sf, &cf);
+        const double q0 = -log(u[2] * u[3]);
+        q[i][0] = q0; q[i][1] = q0 * s * cf; q[i][2] = q0 * s * sf; q[i][3] = q0 * c;
+#pragma unroll
+        for (int mu = 0; mu < 4; ++mu) Q[mu] += q[i][mu];
+    }
+    const double M = sqrt(Q[0] * Q[0] - Q[1] * Q[1] - Q[2] * Q[2] - Q[3] * Q[3]);
+    const double b[3] = {-Q[1] / M, -Q[2] / M, -Q[3] / M};
+    const double gam = Q[0] / M, a = 1.0 / (1.0 + gam), x = rs / M;
+    const double ch = cosh(y), sh = sinh(y);
+
+    double* out = momenta + e * 4 * (N + 2);
+    const double e1 = 0.5 * rs * exp(y), e2 = 0.5 * rs * exp(-y);
+    reinterpret_cast<double2*>(out)[0] = make_double2(e1, 0.0);
+    reinterpret_cast<double2*>(out)[1] = make_double2(0.0, e1);
+    reinterpret_cast<double2*>(out)[2] = make_double2(e2, 0.0);
+    reinterpret_cast<double2*>(out)[3] = make_double2(0.0, -e2);
+
+    bool pass = true;
+    double eta[N], phi[N];
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+        const double bq = b[0] * q[i][1] + b[1] * q[i][2] + b[2] * q[i][3];
+        const double k0 = x * (gam * q[i][0] + bq);
+        const double kx = x * (q[i][1] + b[0] * q[i][0] + a * bq * b[0]);
+        const double ky = x * (q[i][2] + b[1] * q[i][0] + a * bq * b[1]);
+        const double kz = x * (q[i][3] + b[2] * q[i][0] + a * bq * b[2]);
+        const double E = k0 * ch + kz * sh;   // boost by y along z
+        const double pz = kz * ch + k0 * sh;
+        reinterpret_cast<double2*>(out)[4 + 2 * i] = make_double2(E, kx);
+        reinterpret_cast<double2*>(out)[5 + 2 * i] = make_double2(ky, pz);
+        if (cfg.apply_cuts) {
+            const double pt = sqrt(kx * kx + ky * ky);
+            eta[i] = asinh(pz / pt);
+            phi[i] = atan2(ky, kx);
+            pass = pass && (pt > pt_cut) && (fabs(eta[i]) < eta_cut);
+        }
+    }
+    if (cfg.apply_cuts) {
+#pragma unroll
+        for (int i = 0; i < N; ++i)
+#pragma unroll
+            for (int j = i + 1; j < N; ++j) {
+                const double deta = eta[i] - eta[j];
+                double dphi = fabs(phi[i] - phi[j]);
+                if (dphi > pi) dphi = 2.0 * pi - dphi;
+                pass = pass && (sqrt(deta * deta + dphi * dphi) > dr_cut);
+            }
+    }
+    if (weight) {
+        const double shat = rs * rs;
+        weight[e] = pass ? phase_space_volume(N, shat) / (2.0 * shat) * extra : 0.0;
+    }
+}
+
+template <int N>
+cudaError_t launch(const heget_ctx* ctx, uint64_t seed, const heget_gen_cfg& cfg, uint64_t first_event,
+                   int64_t n_events, double* momenta, double* weight, cudaStream_t stream)
+{
+    const int threads = 128;
+    const int64_t blocks = (n_events + threads - 1) / threads;
+    gen_kernel<N><<<(unsigned)blocks, threads, 0, stream>>>(seed, cfg, ctx->pt_cut, ctx->eta_cut, ctx->dr_cut,
+                                                           first_event, n_events, momenta, weight);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+cudaError_t heget_launch_gen(const heget_ctx* ctx, uint64_t seed, int n, const heget_gen_cfg* cfg,
+                             uint64_t first_event, int64_t N, double* momenta, double* weight,
+                             cudaStream_t stream, int* launches)
+{
+    *launches = 0;
+    if (N == 0) return cudaSuccess;
+    *launches = 1;
+    switch (n) {
+        case 2: return launch<2>(ctx, seed, *cfg, first_event, N, momenta, weight, stream);
+        case 3: return launch<3>(ctx, seed, *cfg, first_event, N, momenta, weight, stream);
+        case 4: return launch<4>(ctx, seed, *cfg, first_event, N, momenta, weight, stream);
+        case 5: return launch<5>(ctx, seed, *cfg, first_event, N, momenta, weight, stream);
+        case 6: return launch<6>(ctx, seed, *cfg, first_event, N, momenta, weight, stream);
+        case 7: return launch<7>(ctx, seed, *cfg, first_event, N, momenta, weight, stream);
+        case 8: return launch<8>(ctx, seed, *cfg, first_event, N, momenta, weight, stream);
+        default: return cudaErrorInvalidValue;
+    }
+}

@@ -1,0 +1,38 @@
+// heget_internal.cuh -- shared declarations of libheget.so's translation units (product code).
+// Nothing here is used by, or shared with, oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/heget.h"
+
+struct heget_ctx {
+    int device;
+    int sm_count;
+    double alpha, q_charge;
+    double g;  // gal[0] = gal[1] = -e Q_q (eq. 26)
+    double pt_cut, eta_cut, dr_cut;
+    // scratch owned by the context
+    double* d_partials;     // [kReduceBlocks][3] block partial sums of heget_xsec_reduce
+    double* d_stage_mom;    // staging for the *_host entry point
+    double* d_stage_w;
+    double* d_stage_amp2;
+    double* d_stage_out3;
+    int64_t stage_events;   // capacity of the staging buffers, in events * (n+2)
+    int64_t stage_n_events;
+    cudaStream_t host_stream;
+    int64_t launches;
+    char cuda_msg[256];
+};
+
+constexpr int kReduceBlocks = 296;  // 2 CTAs per SM on a 148-SM B200; any value is correct
+
+// launchers (each returns a cudaError_t from the launch)
+cudaError_t heget_launch_amp2(const heget_ctx* ctx, const double* momenta, int n, int precision,
+                              double* out_amp2, int64_t N, cudaStream_t stream, int* launches);
+cudaError_t heget_launch_gen(const heget_ctx* ctx, uint64_t seed, int n, const heget_gen_cfg* cfg,
+                             uint64_t first_event, int64_t N, double* momenta, double* weight,
+                             cudaStream_t stream, int* launches);
+cudaError_t heget_launch_reduce(const heget_ctx* ctx, const double* amp2, const double* weight, int n,
+                                int64_t N, double* out3, cudaStream_t stream, int* launches);
+cudaError_t heget_run_fma_peak(const heget_ctx* ctx, int precision, double* flops_per_s, int* launches);

@@ -1,0 +1,158 @@
+"""GPU parity: libheget.so (through the C ABI) against the CPU oracle, element by element on
+the same seeded inputs.  Inputs are produced by the oracle's own generator on the host and
+uploaded; nothing the oracle sees comes from the CUDA path.
+
+Tolerances (BASELINE.json north_star): relative error per event <= 1e-12 in fp64 and <= 1e-4 in
+fp32, binding on events that pass the cuts (weight != 0) and on all events of the no-cut
+2-photon config (reading R14); events failing the cuts are still compared, with a
+looser bound, because without the cuts t_S is arbitrarily ill-conditioned."""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_0908_4403_b200 import FP32, FP64, Heget, workloads
+
+pytestmark = pytest.mark.gpu
+
+TOL64, TOL32 = 1e-12, 1e-4
+HEAVY = os.environ.get("HEGET_TEST_HEAVY", "0") == "1"
+
+
+@pytest.fixture(scope="module")
+def hg():
+    h = Heget(0, workloads.ALPHA, workloads.Q_U, workloads.PT_CUT, workloads.ETA_CUT, workloads.DR_CUT)
+    yield h
+    h.close()
+
+
+def oracle_events(name, N, first_event=0):
+    c = workloads.CONFIGS[name]
+    return oracle.gen_events(c["seed"], c["n"], N, mode=c["mode"], a=c["a"], b=c["b"], y_max=c["y_max"],
+                             apply_cuts=c["apply_cuts"], pt_cut=workloads.PT_CUT, eta_cut=workloads.ETA_CUT,
+                             dr_cut=workloads.DR_CUT, first_event=first_event)
+
+
+_ORACLE_CACHE = {}
+
+
+def oracle_amp2_cached(key, mom, extended):
+    """The oracle is expensive for n >= 6: evaluate each input set once per session."""
+    if key not in _ORACLE_CACHE:
+        _ORACLE_CACHE[key] = oracle.amp2(mom, extended=extended)
+    return _ORACLE_CACHE[key]
+
+
+def gpu_amp2(hg, mom, precision):
+    d = torch.from_numpy(mom).cuda()
+    out = hg.amp2(d, precision)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+def report(tag, rel, passing):
+    p = rel[passing] if passing.any() else np.zeros(1)
+    print("\n[parity] %-28s events=%d passing=%d  passing: max=%.3e median=%.3e   all: max=%.3e median=%.3e"
+          % (tag, rel.size, int(passing.sum()), p.max(), np.median(p), rel.max(), np.median(rel)))
+
+
+# sizes: several CTAs plus a ragged tail for every n (events per CTA = 256 / 2^n)
+SMALL = {"2gamma": 64 * 5 + 3, "4gamma": 16 * 9 + 5, "6gamma": 4 * 6 + 1, "7gamma": 5, "8gamma": 2}
+if HEAVY:
+    SMALL.update({"6gamma": 4 * 30 + 1, "7gamma": 24, "8gamma": 6})
+
+
+@pytest.mark.parametrize("name", workloads.ORDER)
+@pytest.mark.parametrize("precision", [FP64, FP32])
+def test_amp2_matches_oracle_on_config_events(hg, name, precision):
+    n = workloads.CONFIGS[name]["n"]
+    N = SMALL[name]
+    mom, w = oracle_events(name, N)
+    if n >= 7:
+        # keep the expensive oracle on events that bind: all cut-passing ones of a larger draw
+        big, wb = oracle_events(name, 200)
+        idx = np.concatenate([np.flatnonzero(wb != 0)[: N - 1], np.flatnonzero(wb == 0)[:1]])
+        mom, w = big[idx], wb[idx]
+    ref = oracle_amp2_cached(name, mom, extended=(n <= 7 or HEAVY))
+    got = gpu_amp2(hg, mom, precision)
+    assert got.shape == ref.shape and np.all(np.isfinite(got)) and np.all(got > 0)
+    rel = np.abs(got / ref - 1.0)
+    passing = (w != 0) if workloads.CONFIGS[name]["apply_cuts"] else np.ones(len(w), bool)
+    report("%s %s" % (name, "fp64" if precision == FP64 else "fp32"), rel, passing)
+    tol = TOL64 if precision == FP64 else TOL32
+    assert passing.sum() >= 1
+    assert np.all(rel[passing] <= tol)
+    assert np.all(rel <= tol * 1e3)          # failing-cut events: reported, loosely bounded
+
+
+@pytest.mark.parametrize("n", [3, 5])
+@pytest.mark.parametrize("precision", [FP64, FP32])
+def test_amp2_matches_oracle_other_multiplicities(hg, n, precision):
+    N = {3: 32 * 4 + 7, 5: 8 * 5 + 3}[n]
+    mom, w = oracle.gen_events(5, n, N, mode=oracle.MODE_LOGUNIFORM, a=300.0, b=4000.0, y_max=1.5,
+                               apply_cuts=True)
+    ref = oracle_amp2_cached("other%d" % n, mom, extended=True)
+    got = gpu_amp2(hg, mom, precision)
+    rel = np.abs(got / ref - 1.0)
+    report("n=%d %s" % (n, "fp64" if precision == FP64 else "fp32"), rel, w != 0)
+    tol = TOL64 if precision == FP64 else TOL32
+    assert np.all(rel[w != 0] <= tol) and np.all(rel <= tol * 1e3)
+
+
+def test_amp2_two_photon_closed_form_fixed_energy(hg):
+    # config 1 as specified: 65,536 events, fixed 1 TeV, no cuts -- all events bind
+    mom, _ = oracle_events("2gamma", 1 << 16)
+    ref = oracle.amp2(mom, extended=True)
+    got = gpu_amp2(hg, mom, FP64)
+    rel = np.abs(got / ref - 1.0)
+    report("2gamma full fp64", rel, np.ones(len(rel), bool))
+    assert np.all(rel <= TOL64)
+    got32 = gpu_amp2(hg, mom, FP32)
+    rel32 = np.abs(got32 / ref - 1.0)
+    report("2gamma full fp32", rel32, np.ones(len(rel), bool))
+    assert np.all(rel32 <= TOL32)
+
+
+@pytest.mark.parametrize("n", [2, 4, 7])
+def test_amp2_edge_sizes(hg, n):
+    mom, _ = oracle.gen_events(9, n, 3, mode=oracle.MODE_FIXED, a=800.0)
+    ref = oracle.amp2(mom)
+    # N = 0: nothing written, no error
+    empty = torch.empty((0, n + 2, 4), dtype=torch.float64, device="cuda")
+    assert hg.amp2(empty).shape == (0,)
+    # N = 1 and a sub-CTA batch
+    for N in (1, 3):
+        got = gpu_amp2(hg, mom[:N], FP64)
+        assert np.all(np.abs(got / ref[:N] - 1.0) < 1e-11)
+    # the output buffer is written only inside [0, N)
+    out = torch.full((5,), -7.0, dtype=torch.float64, device="cuda")
+    hg.amp2(torch.from_numpy(mom).cuda(), FP64, out=out[:3])
+    torch.cuda.synchronize()
+    assert out[3].item() == -7.0 and out[4].item() == -7.0
+
+
+def test_amp2_is_deterministic_and_batch_independent(hg):
+    mom, _ = oracle_events("4gamma", 1000)
+    a = gpu_amp2(hg, mom, FP64)
+    b = gpu_amp2(hg, mom, FP64)
+    assert np.array_equal(a, b)
+    c = gpu_amp2(hg, mom[123:777], FP64)     # different CTA alignment, same per-event result
+    assert np.array_equal(a[123:777], c)
+
+
+def test_invalid_arguments_return_einval(hg):
+    import ctypes
+    lib, ctx = hg._lib, hg._ctx
+    buf = torch.zeros((4, 10, 4), dtype=torch.float64, device="cuda")
+    out = torch.zeros(4, dtype=torch.float64, device="cuda")
+    for n in (1, 9):
+        assert lib.heget_amp2(ctx, buf.data_ptr(), n, FP64, out.data_ptr(), 4, None) == -1
+    assert lib.heget_amp2(ctx, buf.data_ptr(), 4, 7, out.data_ptr(), 4, None) == -1
+    assert lib.heget_amp2(ctx, buf.data_ptr(), 4, FP64, out.data_ptr(), -1, None) == -1
+    assert lib.heget_amp2(ctx, None, 4, FP64, out.data_ptr(), 4, None) == -1
+    assert lib.heget_amp2(ctx, buf.data_ptr() + 8, 4, FP64, out.data_ptr(), 1, None) == -1   # misaligned
+    assert lib.heget_amp2(None, buf.data_ptr(), 4, FP64, out.data_ptr(), 4, None) == -1
+    assert lib.heget_xsec_reduce(ctx, out.data_ptr(), out.data_ptr(), 4, 4, None, None) == -1
+    assert b"invalid" in lib.heget_strerror(-1)
