@@ -38,8 +38,10 @@ def test_gen_events_matches_oracle(hg, name):
     rs = mo[:, 0, 0] + mo[:, 1, 0]                      # scale of every component
     err = np.abs(mg - mo).max(axis=(1, 2)) / rs
     print("\n[gen parity] %s: momenta max rel %.3e median %.3e" % (name, err.max(), np.median(err)))
-    # device log/sincos/pow differ from libm by ulps; RAMBO's boost amplifies that by gamma^2
-    assert np.median(err) < 1e-15 and err.max() < 1e-11
+    # device log/sincos/pow differ from libm by ulps; RAMBO's conformal boost amplifies an ulp
+    # by gamma^2 = (Q0/M)^2, unbounded for nearly collinear q_i (worst for n = 2), so the bound
+    # is on quantiles plus a loose cap
+    assert np.median(err) < 1e-15 and np.quantile(err, 0.999) < 1e-12 and err.max() < 1e-9
     # cut decisions: identical except where an observable sits within 1e-9 of a threshold
     same = (wo != 0) == (wg != 0)
     assert same.mean() == 1.0 or (~same).sum() <= 1
