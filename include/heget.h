@@ -122,6 +122,15 @@ int heget_xsec_host(heget_ctx* ctx, const double* momenta, const double* weight,
  * writes the achieved FLOP/s (FMA = 2) to *flops_per_s [host].  Synchronises. */
 int heget_fma_peak(heget_ctx* ctx, int precision, double* flops_per_s);
 
+/* The same measurement for other operand patterns (context for the roofline: the amplitude
+ * kernels' FMAs take three register operands, which the register file cannot feed at the
+ * pipe's peak rate):
+ *   HEGET_PEAK_CONST_OPERAND  x = x*a + b, a and b constant-bank operands (= heget_fma_peak)
+ *   HEGET_PEAK_THREE_REG      x = y*z + x, three distinct registers, no operand reuse
+ *   HEGET_PEAK_NODE_PATTERN   the fvixx0 node (16 FMA + 4 MUL per node, 36 flop) on registers */
+enum { HEGET_PEAK_CONST_OPERAND = 0, HEGET_PEAK_THREE_REG = 1, HEGET_PEAK_NODE_PATTERN = 2 };
+int heget_fma_peak_pattern(heget_ctx* ctx, int precision, int pattern, double* flops_per_s);
+
 /* Number of kernel launches this context has issued (all entry points), for bench.py's
  * gpu_launches count. */
 int64_t heget_launch_count(const heget_ctx* ctx);

@@ -15,7 +15,7 @@ FP32, FP64 = 0, 1
 GEN_FIXED, GEN_LOGUNIFORM, GEN_TOYPDF = 0, 1, 2
 
 EXPORTS = ["heget_init", "heget_destroy", "heget_strerror", "heget_last_cuda_error", "heget_rambo",
-           "heget_gen_events", "heget_amp2", "heget_xsec_reduce", "heget_xsec_host", "heget_fma_peak",
+           "heget_gen_events", "heget_amp2", "heget_xsec_reduce", "heget_xsec_host", "heget_fma_peak", "heget_fma_peak_pattern",
            "heget_launch_count"]
 
 
@@ -62,6 +62,8 @@ def load_library():
     lib.heget_xsec_host.restype = ci
     lib.heget_fma_peak.argtypes = [vp, ci, ctypes.POINTER(cd)]
     lib.heget_fma_peak.restype = ci
+    lib.heget_fma_peak_pattern.argtypes = [vp, ci, ci, ctypes.POINTER(cd)]
+    lib.heget_fma_peak_pattern.restype = ci
     lib.heget_launch_count.argtypes = [vp]
     lib.heget_launch_count.restype = i64
     _lib = lib
@@ -163,9 +165,10 @@ class Heget:
                                               N, amp_ptr, out3.data_ptr()), "heget_xsec_host")
         return out3
 
-    def fma_peak(self, precision):
+    def fma_peak(self, precision, pattern=0):
         v = ctypes.c_double()
-        self._check(self._lib.heget_fma_peak(self._ctx, precision, ctypes.byref(v)), "heget_fma_peak")
+        self._check(self._lib.heget_fma_peak_pattern(self._ctx, precision, pattern, ctypes.byref(v)),
+                    "heget_fma_peak_pattern")
         return v.value
 
     def launch_count(self):

@@ -14,6 +14,19 @@
 #include "amp2_tables.cuh"
 #include "heget_internal.cuh"
 
+#ifndef HEGET_KB
+#define HEGET_KB 4          // unrolled bottom levels of the permutation tree
+#endif
+#ifndef HEGET_E_BY_PTR
+#define HEGET_E_BY_PTR 0    // 1: Bottom<K> re-reads E' entries from shared memory instead of holding them
+#endif
+#ifndef HEGET_MINB32
+#define HEGET_MINB32 1      // __launch_bounds__ min CTAs per SM, fp32 / fp64 kernels
+#endif
+#ifndef HEGET_MINB64
+#define HEGET_MINB64 2
+#endif
+
 namespace {
 
 template <typename T>
@@ -21,50 +34,105 @@ struct Spinor {
     T r0, i0, r1, i1;  // two complex components
 };
 
-// fvixx0 in Weyl form: psi' = P_S * (E_i * psi).
+// fvixx0 in Weyl form: psi' = P_S * (E'_i * psi), 20 FMA-pipe instructions.
 template <typename T>
 __device__ __forceinline__ Spinor<T> fvixx0_weyl(const PEntry<T>& P, const EEntry<T>& E, const Spinor<T>& f)
 {
-    // w = E f,  E = [[-s, -B], [A, s]]
-    const T w0r = -E.s * f.r0 - (E.br * f.r1 - E.bi * f.i1);
-    const T w0i = -E.s * f.i0 - (E.br * f.i1 + E.bi * f.r1);
-    const T w1r = E.s * f.r1 + (E.ar * f.r0 - E.ai * f.i0);
-    const T w1i = E.s * f.i1 + (E.ar * f.i0 + E.ai * f.r0);
+    // w = E' f,  E' = [[-1, -b], [a, 1]]
+    const T w0r = fma(-E.br, f.r1, fma(E.bi, f.i1, -f.r0));
+    const T w0i = fma(-E.br, f.i1, fma(-E.bi, f.r1, -f.i0));
+    const T w1r = fma(E.ar, f.r0, fma(-E.ai, f.i0, f.r1));
+    const T w1i = fma(E.ar, f.i0, fma(E.ai, f.r0, f.i1));
     // psi' = P w,  P = [[pp, px - i py], [px + i py, pm]]
     Spinor<T> o;
-    o.r0 = P.pp * w0r + (P.px * w1r + P.py * w1i);
-    o.i0 = P.pp * w0i + (P.px * w1i - P.py * w1r);
-    o.r1 = P.pm * w1r + (P.px * w0r - P.py * w0i);
-    o.i1 = P.pm * w1i + (P.px * w0i + P.py * w0r);
+    o.r0 = fma(P.pp, w0r, fma(P.px, w1r, P.py * w1i));
+    o.i0 = fma(P.pp, w0i, fma(P.px, w1i, -(P.py * w1r)));
+    o.r1 = fma(P.pm, w1r, fma(P.px, w0r, -(P.py * w0i)));
+    o.i1 = fma(P.pm, w1i, fma(P.px, w0i, P.py * w0r));
     return o;
 }
 
 // iovxxx in Weyl form: vbar (oxxxx2) has the single component 1 of the (0,1)
-// pair, so amp = row 1 of E_j times psi = A psi0 + s psi1 (constant factors applied at the end).
+// pair, so amp = row 1 of E'_j times psi = a psi0 + psi1 (constant factors applied at the end).
 template <typename T>
 __device__ __forceinline__ void iovxxx_weyl(const EEntry<T>& E, const Spinor<T>& f, T& ar, T& ai)
 {
-    ar += E.s * f.r1 + (E.ar * f.r0 - E.ai * f.i0);
-    ai += E.s * f.i1 + (E.ar * f.i0 + E.ai * f.r0);
+    ar += fma(E.ar, f.r0, fma(-E.ai, f.i0, f.r1));
+    ai += fma(E.ar, f.i0, fma(E.ai, f.r0, f.i1));
 }
 
-// Depth-first walk.  `used` = set of photons already attached (uniform over the CTA).
-template <int N, int DEPTH, typename T>
+// Bottom K levels of the permutation tree, fully unrolled.  The K photons still to attach are
+// held as compile-time-indexed register arrays (bit[] = their subset-index bits, e[] = this
+// lane's E' entries), so choosing a child is register renaming, not bit arithmetic: the code
+// of a subtree is straight-line FMAs plus one P-entry load per node.
+template <typename T> __device__ __forceinline__ const EEntry<T>& eload(const EEntry<T>& e) { return e; }
+template <typename T> __device__ __forceinline__ EEntry<T> eload(const EEntry<T>* e) { return *e; }
+
+template <int K, typename T, typename EA>
+struct Bottom {
+    static __device__ __forceinline__ void run(const PEntry<T>* __restrict__ PS, const int (&bit)[K],
+                                               const EA (&e)[K], const Spinor<T>& f, T& ar, T& ai)
+    {
+#pragma unroll
+        for (int i = 0; i < K; ++i) {
+            int sub_bit[K - 1];
+            EA sub_e[K - 1];
+#pragma unroll
+            for (int m = 0; m < K - 1; ++m) {
+                sub_bit[m] = bit[m + (m >= i ? 1 : 0)];
+                sub_e[m] = e[m + (m >= i ? 1 : 0)];
+            }
+            const PEntry<T>* Pn = PS + bit[i];
+            const Spinor<T> fn = fvixx0_weyl(*Pn, eload<T>(e[i]), f);
+            Bottom<K - 1, T, EA>::run(Pn, sub_bit, sub_e, fn, ar, ai);
+        }
+    }
+};
+
+template <typename T, typename EA>
+struct Bottom<1, T, EA> {
+    static __device__ __forceinline__ void run(const PEntry<T>* __restrict__, const int (&)[1],
+                                               const EA (&e)[1], const Spinor<T>& f, T& ar, T& ai)
+    {
+        iovxxx_weyl(eload<T>(e[0]), f, ar, ai);
+    }
+};
+
+// Depth-first walk of the upper levels.  `used` = set of photons already attached (uniform
+// over the CTA); when KB photons remain the unrolled Bottom<KB> takes over.
+template <int N, int DEPTH, int KB, typename T>
 struct Walk {
     static __device__ __forceinline__ void run(const PEntry<T>* __restrict__ P, const EEntry<T>* __restrict__ E,
                                                unsigned hel, unsigned used, const Spinor<T>& f, T& ar, T& ai)
     {
         unsigned avail = ((1u << N) - 1u) & ~used;
-        if constexpr (DEPTH == N - 1) {
-            const int j = __ffs(avail) - 1;
-            iovxxx_weyl(E[2 * j + ((hel >> j) & 1u)], f, ar, ai);
+        if constexpr (N - DEPTH == KB) {
+            int bit[KB];
+#if HEGET_E_BY_PTR
+            using EA = const EEntry<T>*;
+#else
+            using EA = EEntry<T>;
+#endif
+            EA e[KB];
+#pragma unroll
+            for (int m = 0; m < KB; ++m) {
+                const int i = __ffs(avail) - 1;
+                avail &= avail - 1u;
+                bit[m] = 1 << i;
+#if HEGET_E_BY_PTR
+                e[m] = &E[2 * i + ((hel >> i) & 1u)];
+#else
+                e[m] = E[2 * i + ((hel >> i) & 1u)];
+#endif
+            }
+            Bottom<KB, T, EA>::run(P + used, bit, e, f, ar, ai);
         } else {
             while (avail) {
                 const int i = __ffs(avail) - 1;
                 avail &= avail - 1u;
                 const unsigned S = used | (1u << i);
                 const Spinor<T> fn = fvixx0_weyl(P[S], E[2 * i + ((hel >> i) & 1u)], f);
-                Walk<N, DEPTH + 1, T>::run(P, E, hel, S, fn, ar, ai);
+                Walk<N, DEPTH + 1, KB, T>::run(P, E, hel, S, fn, ar, ai);
             }
         }
     }
@@ -75,10 +143,11 @@ struct Geometry {
     static constexpr int L = 1 << N;                       // lanes (helicity configurations) per event
     static constexpr int THREADS = (L > 256) ? L : 256;
     static constexpr int EPB = THREADS / L;                // events per CTA
+    static constexpr int KB = (N < HEGET_KB) ? N : HEGET_KB;             // unrolled bottom levels of the tree
 };
 
 template <int N, typename T>
-__global__ void __launch_bounds__(Geometry<N>::THREADS)
+__global__ void __launch_bounds__(Geometry<N>::THREADS, (sizeof(T) == 4) ? HEGET_MINB32 : HEGET_MINB64)
 amp2_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_t n_events, double g)
 {
     using G = Geometry<N>;
@@ -87,6 +156,7 @@ amp2_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_
     __shared__ PEntry<T> s_P[G::EPB * G::L];
     __shared__ EEntry<T> s_E[G::EPB * 2 * N];
     __shared__ double s_red[G::THREADS / 32];
+    __shared__ double s_s2[G::EPB * N];  // s_i^2 = (pT/w)^2 taken out of photon i's E entries
 
     const int tid = threadIdx.x;
     const int ev_local = tid / G::L;
@@ -110,17 +180,21 @@ amp2_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_
     const double scale = (sizeof(T) == 4) ? sqrt(shat) : 1.0;
     // a4: vxxxx0 for both helicities of photon `hel` (lanes 0..N-1 of each event)
     if (hel < (unsigned)N)
-        make_photon_entries<T>(mom + 4 * (2 + hel), &s_E[(ev_local * N + hel) * 2 + 1],
-                               &s_E[(ev_local * N + hel) * 2 + 0]);
+        s_s2[ev_local * N + hel] = make_photon_entries<T>(mom + 4 * (2 + hel), &s_E[(ev_local * N + hel) * 2 + 1],
+                                                          &s_E[(ev_local * N + hel) * 2 + 0]);
     // a5: subset kinematics, one subset per lane
-    if (hel >= 1u && hel <= (unsigned)(G::L - 2))
-        make_subset_entry<N, T>(mom, hel, g, scale, &s_P[ev_local * G::L + hel]);
+    if (hel >= 1u && hel <= (unsigned)(G::L - 2)) {
+        if constexpr (sizeof(T) == 4)
+            make_subset_entry_plain<N>(mom, hel, g, scale, &s_P[ev_local * G::L + hel]);
+        else
+            make_subset_entry<N, T>(mom, hel, g, scale, &s_P[ev_local * G::L + hel]);
+    }
     __syncthreads();
 
     // a2, a6, a7: psi_0 = u(p1,+)/sqrt(2E1) = (1,0); walk the permutation tree
     T ar = 0, ai = 0;
     const Spinor<T> f0 = {(T)1, (T)0, (T)0, (T)0};
-    Walk<N, 0, T>::run(s_P + ev_local * G::L, s_E + ev_local * 2 * N, hel, 0u, f0, ar, ai);
+    Walk<N, 0, G::KB, T>::run(s_P + ev_local * G::L, s_E + ev_local * 2 * N, hel, 0u, f0, ar, ai);
 
     // a8: |ampsum|^2 summed over the event's 2^N lanes
     double m2 = (double)ar * (double)ar + (double)ai * (double)ai;
@@ -138,10 +212,11 @@ amp2_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_
     }
     if (hel == 0 && ev0 + ev_local < n_events) {
         // constants: 2 (parity) * g^2 (closing vertex) * 2E1*2E2 = s_hat (spinor norms) * 2^-N
-        // (the sqrt(2) of every polarisation vector); fp32 worked in units of sqrt(s_hat)
+        // (the sqrt(2) of every polarisation vector) * prod s_i^2 (E' normalisation);
+        // fp32 worked in units of sqrt(s_hat)
         double f = 2.0 * g * g * shat;
 #pragma unroll
-        for (int i = 0; i < N; ++i) f *= 0.5;
+        for (int i = 0; i < N; ++i) f *= 0.5 * s_s2[ev_local * N + i];
         if (sizeof(T) == 4) {
             const double inv = 1.0 / shat;
 #pragma unroll

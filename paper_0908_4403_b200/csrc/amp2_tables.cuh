@@ -9,10 +9,16 @@
 // chain lives in two complex components.  The paper keeps 4-spinors
 // (the gain "never exceeds a factor of two"); here that factor is taken.
 //
-// E table, per photon i and helicity lambda (vxxxx0, eqs. 13-15, nSV=+1),
-// upper-right block of eps-slash times sqrt(2):
-//     lambda=+1: [[-s, -B], [A, s]],  s = pT/w, A = (1+c) e^{i phi}, B = (1-c) e^{-i phi}
+// E table, per photon i and helicity lambda (vxxxx0, eqs. 13-15, nSV=+1):
+// the upper-right block of eps-slash times sqrt(2) is, with s = pT/w = sin(theta),
+//     lambda=+1: [[-s, -B], [A, s]],  A = (1+c) e^{i phi}, B = (1-c) e^{-i phi}
 //     lambda=-1: same form with s -> -s, A -> conj(B), B -> conj(A)   (eps(-l) = -eps(l)^*)
+// Every diagram of a helicity configuration contains each photon exactly once, so a factor
+// common to all four elements of photon i's block is a factor of ampsum.  The table stores
+// the block divided by +s (lambda=+1) or -s (lambda=-1),
+//     E' = [[-1, -b], [a, 1]],   a = A/s, b = B/s   (lambda=-1: a = -conj(B)/s, b = -conj(A)/s)
+// i.e. four reals per entry and no multiplications by s in the tree; |ampsum|^2 is multiplied
+// by prod_i s_i^2 (helicity independent) once per event, in fp64.
 // P table, per non-empty proper subset S of photons (eq. 8), lower-left block of
 // (p1 - K_S)-slash times the propagator factor -g/t_S of fvixx0:
 //     (-g/t_S) * [[p+, px - i py], [px + i py, p-]],  p+- = p0 +- p3 of p1 - K_S.
@@ -21,8 +27,7 @@
 
 template <typename T>
 struct alignas(16) EEntry {
-    T s, ar, ai, br;
-    T bi, pad0, pad1, pad2;
+    T ar, ai, br, bi;
 };
 
 template <typename T>
@@ -30,21 +35,63 @@ struct alignas(16) PEntry {
     T pp, pm, px, py;
 };
 
-// Photon i's two E entries from its four-momentum k = (w, kx, ky, kz), in fp64.
+// 1/x for a normal, finite double: hardware approximation (>= 20 bits) and two Newton steps,
+// without the slow path of the IEEE division (the tables never see 0, inf or subnormals for
+// inputs that satisfy the preconditions of include/heget.h).  Relative error ~1 ulp.
+__device__ __forceinline__ double fast_rcp(double x)
+{
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    r = fma(r, fma(-x, r, 1.0), r);
+    r = fma(r, fma(-x, r, 1.0), r);
+    return r;
+}
+
+// Photon i's two E' entries from its four-momentum k = (w, kx, ky, kz), in fp64.
+// Returns s^2 = (pT/w)^2, the factor taken out of |ampsum|^2.
 template <typename T>
-__device__ __forceinline__ void make_photon_entries(const double* k, EEntry<T>* e_plus, EEntry<T>* e_minus)
+__device__ __forceinline__ double make_photon_entries(const double* k, EEntry<T>* e_plus, EEntry<T>* e_minus)
 {
     const double w = k[0], kx = k[1], ky = k[2], kz = k[3];
-    const double pt = sqrt(kx * kx + ky * ky);
-    const double inv_w = 1.0 / w, inv_pt = 1.0 / pt;
-    const double opc = (w + kz) * inv_w;  // 1 + cos(theta)
-    const double omc = (w - kz) * inv_w;  // 1 - cos(theta): one rounded subtraction, no 1 - c
-    const double s = pt * inv_w;
-    const double cf = kx * inv_pt, sf = ky * inv_pt;
-    const double ar = opc * cf, ai = opc * sf;   // A = (1+c) e^{+i phi}
-    const double br = omc * cf, bi = -omc * sf;  // B = (1-c) e^{-i phi}
-    e_plus->s = (T)s;   e_plus->ar = (T)ar;  e_plus->ai = (T)ai;   e_plus->br = (T)br;  e_plus->bi = (T)bi;
-    e_minus->s = (T)-s; e_minus->ar = (T)br; e_minus->ai = (T)-bi; e_minus->br = (T)ar; e_minus->bi = (T)-ai;
+    const double pt2 = kx * kx + ky * ky;
+    const double w2 = w * w;
+    const double r = fast_rcp(pt2 * w2);  // one reciprocal serves 1/pT^2 and pT^2/w^2
+    const double inv_pt2 = r * w2;
+    const double ca = (w + kz) * inv_pt2;  // (1+c)/s / pT
+    const double cb = (w - kz) * inv_pt2;  // (1-c)/s / pT: one rounded subtraction, no 1 - c
+    const double ar = ca * kx, ai = ca * ky;    // a = (1+c)/s e^{+i phi}
+    const double br = cb * kx, bi = -cb * ky;   // b = (1-c)/s e^{-i phi}
+    e_plus->ar = (T)ar;   e_plus->ai = (T)ai;  e_plus->br = (T)br;   e_plus->bi = (T)bi;
+    e_minus->ar = (T)-br; e_minus->ai = (T)bi; e_minus->br = (T)-ar; e_minus->bi = (T)ai;
+    return pt2 * pt2 * r;
+}
+
+// P entry of subset S for the fp32 kernel, in plain fp64 and rounded to fp32 once: light-cone
+// components k+- = w +- kz of each photon (one rounded operation each), p+ = 2 E1 - sum k+,
+// p- = -sum k-, t_S = p+ p- - px^2 - py^2 (both terms <= 0, no cancellation between them).
+// Error ~1e-13 relative on cut-passing events, far below fp32's 6e-8.
+template <int N>
+__device__ __forceinline__ void make_subset_entry_plain(const double* mom, unsigned S, double g, double scale,
+                                                        PEntry<float>* out)
+{
+    double kp = 0.0, km = 0.0, kx = 0.0, ky = 0.0;
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+        if ((S >> i) & 1u) {
+            const double* k = mom + 4 * (2 + i);
+            kp += k[0] + k[3];
+            km += k[0] - k[3];
+            kx += k[1];
+            ky += k[2];
+        }
+    }
+    const double pp = 2.0 * mom[0] - kp;
+    const double t = -fma(pp, km, fma(kx, kx, ky * ky));
+    const double c = -g * scale * fast_rcp(t);
+    out->pp = (float)(c * pp);
+    out->pm = (float)(-c * km);
+    out->px = (float)(-c * kx);
+    out->py = (float)(-c * ky);
 }
 
 // P entry of subset S (bit i set = photon i attached).  mom: the event's (n+2) four-vectors.
@@ -71,7 +118,7 @@ __device__ __forceinline__ void make_subset_entry(const double* mom, unsigned S,
     dd t = dd_mul(pp, pm);
     t = dd_add(t, dd_neg(dd_mul(px, px)));
     t = dd_add(t, dd_neg(dd_mul(py, py)));
-    const double c = -g / dd_to_double(t) * scale;
+    const double c = -g * scale * fast_rcp(dd_to_double(t));
     out->pp = (T)(c * dd_to_double(pp));
     out->pm = (T)(c * dd_to_double(pm));
     out->px = (T)(c * dd_to_double(px));

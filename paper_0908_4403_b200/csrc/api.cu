@@ -197,11 +197,17 @@ int heget_xsec_host(heget_ctx* ctx, const double* momenta, const double* weight,
 
 int heget_fma_peak(heget_ctx* ctx, int precision, double* flops_per_s)
 {
+    return heget_fma_peak_pattern(ctx, precision, HEGET_PEAK_CONST_OPERAND, flops_per_s);
+}
+
+int heget_fma_peak_pattern(heget_ctx* ctx, int precision, int pattern, double* flops_per_s)
+{
     if (!ctx || !flops_per_s || (precision != HEGET_FP32 && precision != HEGET_FP64)) return HEGET_EINVAL;
+    if (pattern < HEGET_PEAK_CONST_OPERAND || pattern > HEGET_PEAK_NODE_PATTERN) return HEGET_EINVAL;
     DeviceGuard guard(ctx->device);
     if (!guard.ok) return fail_cuda(ctx, cudaGetLastError());
     int launches = 0;
-    cudaError_t err = heget_run_fma_peak(ctx, precision, flops_per_s, &launches);
+    cudaError_t err = heget_run_fma_peak(ctx, precision, pattern, flops_per_s, &launches);
     ctx->launches += launches;
     return err == cudaSuccess ? HEGET_OK : fail_cuda(ctx, err);
 }

@@ -35,4 +35,4 @@ cudaError_t heget_launch_gen(const heget_ctx* ctx, uint64_t seed, int n, const h
                              cudaStream_t stream, int* launches);
 cudaError_t heget_launch_reduce(const heget_ctx* ctx, const double* amp2, const double* weight, int n,
                                 int64_t N, double* out3, cudaStream_t stream, int* launches);
-cudaError_t heget_run_fma_peak(const heget_ctx* ctx, int precision, double* flops_per_s, int* launches);
+cudaError_t heget_run_fma_peak(const heget_ctx* ctx, int precision, int pattern, double* flops_per_s, int* launches);
