@@ -100,6 +100,19 @@ int heget_gen_events(heget_ctx* ctx, uint64_t seed, int n, const heget_gen_cfg* 
 int heget_amp2(heget_ctx* ctx, const double* momenta, int n, int precision, double* out_amp2,
                int64_t N, void* stream);
 
+/* The same quantity with a selectable organisation of the permutation sum:
+ *   HEGET_ALGO_TREE    depth-first permutation tree with prefix reuse (= heget_amp2; the method
+ *                      of eq. 6 / List 2)
+ *   HEGET_ALGO_SUBSET  recursion over photon subsets: Psi(S) = P_S sum_{i in S} E_i Psi(S\i); the
+ *                      propagators of eq. (8) depend on the set S only, so the n! orderings
+ *                      collapse onto 2^n sets (3^n - 1 spinors per event including helicities).
+ *                      Same result up to rounding order; NOT the permutation-tree method, hence a
+ *                      separately named mode (reuse of off-shell lines).
+ * Arguments, layout and errors as heget_amp2; algo outside the enum gives HEGET_EINVAL. */
+enum { HEGET_ALGO_TREE = 0, HEGET_ALGO_SUBSET = 1 };
+int heget_amp2_algo(heget_ctx* ctx, const double* momenta, int n, int precision, int algo,
+                    double* out_amp2, int64_t N, void* stream);
+
 /* Step 6 of PAPER.md:141 on the device: with x_e = weight[e] * amp2[e] * (1/4)(1/9)(1/n!)
  * (helicity average, colour factor and identical-photon factor of eq. 2, PAPER.md:37;
  * DESIGN.md R1 for the colour factor),

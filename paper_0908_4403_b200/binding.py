@@ -12,10 +12,11 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libheget.so")
 
 FP32, FP64 = 0, 1
+ALGO_TREE, ALGO_SUBSET = 0, 1
 GEN_FIXED, GEN_LOGUNIFORM, GEN_TOYPDF = 0, 1, 2
 
 EXPORTS = ["heget_init", "heget_destroy", "heget_strerror", "heget_last_cuda_error", "heget_rambo",
-           "heget_gen_events", "heget_amp2", "heget_xsec_reduce", "heget_xsec_host", "heget_fma_peak", "heget_fma_peak_pattern",
+           "heget_gen_events", "heget_amp2", "heget_amp2_algo", "heget_xsec_reduce", "heget_xsec_host", "heget_fma_peak", "heget_fma_peak_pattern",
            "heget_launch_count"]
 
 
@@ -56,6 +57,8 @@ def load_library():
     lib.heget_gen_events.restype = ci
     lib.heget_amp2.argtypes = [vp, dp, ci, ci, dp, i64, vp]
     lib.heget_amp2.restype = ci
+    lib.heget_amp2_algo.argtypes = [vp, dp, ci, ci, ci, dp, i64, vp]
+    lib.heget_amp2_algo.restype = ci
     lib.heget_xsec_reduce.argtypes = [vp, dp, dp, ci, i64, dp, vp]
     lib.heget_xsec_reduce.restype = ci
     lib.heget_xsec_host.argtypes = [vp, dp, dp, ci, ci, i64, dp, dp]
@@ -129,7 +132,7 @@ class Heget:
                                                _stream_ptr(self.device)), "heget_gen_events")
         return momenta, weight
 
-    def amp2(self, momenta, precision=FP64, out=None):
+    def amp2(self, momenta, precision=FP64, out=None, algo=ALGO_TREE):
         _check_dev(momenta, None, self.device)
         if momenta.dim() != 3 or momenta.shape[2] != 4:
             raise HegetError("momenta must be [N][n+2][4]")
@@ -137,8 +140,8 @@ class Heget:
         if out is None:
             out = torch.empty((N,), dtype=torch.float64, device=self.device)
         _check_dev(out, (N,), self.device)
-        self._check(self._lib.heget_amp2(self._ctx, momenta.data_ptr(), n, precision, out.data_ptr(), N,
-                                         _stream_ptr(self.device)), "heget_amp2")
+        self._check(self._lib.heget_amp2_algo(self._ctx, momenta.data_ptr(), n, precision, algo, out.data_ptr(), N,
+                                              _stream_ptr(self.device)), "heget_amp2_algo")
         return out
 
     def xsec_reduce(self, amp2, weight, n, out3=None):

@@ -11,8 +11,7 @@
 // iovxxx accumulated into ampsum (List 2).
 // Only sigma_1 = +1, sigma_2 = -1 is evaluated: sigma_1 = sigma_2 vanishes identically and
 // |M(-sigma,-lambda)| = |M(sigma,lambda)|, so the helicity sum is twice the sum over lambda.
-#include "amp2_tables.cuh"
-#include "heget_internal.cuh"
+#include "amp2_common.cuh"
 
 #ifndef HEGET_KB
 #define HEGET_KB 4          // unrolled bottom levels of the permutation tree
@@ -28,11 +27,6 @@
 #endif
 
 namespace {
-
-template <typename T>
-struct Spinor {
-    T r0, i0, r1, i1;  // two complex components
-};
 
 // fvixx0 in Weyl form: psi' = P_S * (E'_i * psi), 20 FMA-pipe instructions.
 template <typename T>
@@ -139,12 +133,7 @@ struct Walk {
 };
 
 template <int N>
-struct Geometry {
-    static constexpr int L = 1 << N;                       // lanes (helicity configurations) per event
-    static constexpr int THREADS = (L > 256) ? L : 256;
-    static constexpr int EPB = THREADS / L;                // events per CTA
-    static constexpr int KB = (N < HEGET_KB) ? N : HEGET_KB;             // unrolled bottom levels of the tree
-};
+constexpr int kBottom = (N < HEGET_KB) ? N : HEGET_KB;  // unrolled bottom levels of the tree
 
 template <int N, typename T>
 __global__ void __launch_bounds__(Geometry<N>::THREADS, (sizeof(T) == 4) ? HEGET_MINB32 : HEGET_MINB64)
@@ -158,72 +147,19 @@ amp2_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_
     __shared__ double s_red[G::THREADS / 32];
     __shared__ double s_s2[G::EPB * N];  // s_i^2 = (pT/w)^2 taken out of photon i's E entries
 
-    const int tid = threadIdx.x;
-    const int ev_local = tid / G::L;
-    const unsigned hel = tid % G::L;
-    const int64_t ev0 = (int64_t)blockIdx.x * G::EPB;
+    const int ev_local = threadIdx.x / G::L;
+    const unsigned hel = threadIdx.x % G::L;
 
-    // a1: coalesced load of the CTA's momenta (events past the end re-read the last event)
-    {
-        const double2* src = reinterpret_cast<const double2*>(momenta);
-        double2* dst = reinterpret_cast<double2*>(s_mom);
-        for (int idx = tid; idx < G::EPB * MOM / 2; idx += G::THREADS) {
-            int64_t e = ev0 + idx / (MOM / 2);
-            if (e >= n_events) e = n_events - 1;
-            dst[idx] = src[e * (MOM / 2) + idx % (MOM / 2)];
-        }
-    }
-    __syncthreads();
-
-    const double* mom = s_mom + ev_local * MOM;
-    const double shat = 4.0 * mom[0] * mom[4];  // (p1+p2)^2 for p1 || +z, p2 || -z
-    const double scale = (sizeof(T) == 4) ? sqrt(shat) : 1.0;
-    // a4: vxxxx0 for both helicities of photon `hel` (lanes 0..N-1 of each event)
-    if (hel < (unsigned)N)
-        s_s2[ev_local * N + hel] = make_photon_entries<T>(mom + 4 * (2 + hel), &s_E[(ev_local * N + hel) * 2 + 1],
-                                                          &s_E[(ev_local * N + hel) * 2 + 0]);
-    // a5: subset kinematics, one subset per lane
-    if (hel >= 1u && hel <= (unsigned)(G::L - 2)) {
-        if constexpr (sizeof(T) == 4)
-            make_subset_entry_plain<N>(mom, hel, g, scale, &s_P[ev_local * G::L + hel]);
-        else
-            make_subset_entry<N, T>(mom, hel, g, scale, &s_P[ev_local * G::L + hel]);
-    }
-    __syncthreads();
+    // a1, a4, a5: momenta -> shared memory, E' and P tables of the CTA's events
+    build_event_tables<N, T>(momenta, n_events, g, s_mom, s_P, s_E, s_s2);
 
     // a2, a6, a7: psi_0 = u(p1,+)/sqrt(2E1) = (1,0); walk the permutation tree
     T ar = 0, ai = 0;
     const Spinor<T> f0 = {(T)1, (T)0, (T)0, (T)0};
-    Walk<N, 0, G::KB, T>::run(s_P + ev_local * G::L, s_E + ev_local * 2 * N, hel, 0u, f0, ar, ai);
+    Walk<N, 0, kBottom<N>, T>::run(s_P + ev_local * G::L, s_E + ev_local * 2 * N, hel, 0u, f0, ar, ai);
 
-    // a8: |ampsum|^2 summed over the event's 2^N lanes
-    double m2 = (double)ar * (double)ar + (double)ai * (double)ai;
-    constexpr int WL = (G::L < 32) ? G::L : 32;
-#pragma unroll
-    for (int off = WL / 2; off > 0; off >>= 1) m2 += __shfl_xor_sync(0xffffffffu, m2, off);
-    if constexpr (G::L > 32) {
-        if ((tid & 31) == 0) s_red[tid >> 5] = m2;
-        __syncthreads();
-        if (hel == 0) {
-            m2 = 0.0;
-#pragma unroll
-            for (int w = 0; w < G::L / 32; ++w) m2 += s_red[ev_local * (G::L / 32) + w];
-        }
-    }
-    if (hel == 0 && ev0 + ev_local < n_events) {
-        // constants: 2 (parity) * g^2 (closing vertex) * 2E1*2E2 = s_hat (spinor norms) * 2^-N
-        // (the sqrt(2) of every polarisation vector) * prod s_i^2 (E' normalisation);
-        // fp32 worked in units of sqrt(s_hat)
-        double f = 2.0 * g * g * shat;
-#pragma unroll
-        for (int i = 0; i < N; ++i) f *= 0.5 * s_s2[ev_local * N + i];
-        if (sizeof(T) == 4) {
-            const double inv = 1.0 / shat;
-#pragma unroll
-            for (int i = 0; i < N - 1; ++i) f *= inv;
-        }
-        out[ev0 + ev_local] = f * m2;
-    }
+    // a8: |ampsum|^2 summed over the event's 2^N lanes, constant factors, store
+    finish_event<N, T>(ar, ai, s_mom, s_s2, s_red, g, out, n_events);
 }
 
 template <int N, typename T>

@@ -1,0 +1,102 @@
+// amp2_common.cuh -- what the amplitude kernels (amp2.cu: permutation tree; amp2_subset.cu:
+// subset recursion) share: thread geometry, the per-event prologue that fills the E' and P
+// tables in shared memory, and the epilogue that squares, sums over helicities and stores
+// (product code).
+#pragma once
+#include "amp2_tables.cuh"
+#include "heget_internal.cuh"
+
+template <typename T>
+struct alignas(16) Spinor {
+    T r0, i0, r1, i1;  // two complex components
+};
+
+// One lane per photon-helicity configuration: 2^N lanes per event, 256-thread CTAs.
+template <int N>
+struct Geometry {
+    static constexpr int L = 1 << N;                       // lanes (helicity configurations) per event
+    static constexpr int THREADS = (L > 256) ? L : 256;
+    static constexpr int EPB = THREADS / L;                // events per CTA
+};
+
+// a1: coalesced double2 load of the CTA's momenta (events past the end re-read the last
+// event); a4: vxxxx0 for both helicities of photon `hel` (lanes 0..N-1 of each event);
+// a5: subset kinematics, one subset per lane.  Ends with a CTA barrier.
+template <int N, typename T>
+__device__ __forceinline__ void build_event_tables(const double* __restrict__ momenta, int64_t n_events, double g,
+                                                   double* s_mom, PEntry<T>* s_P, EEntry<T>* s_E, double* s_s2)
+{
+    using G = Geometry<N>;
+    constexpr int MOM = 4 * (N + 2);
+    const int tid = threadIdx.x;
+    const int ev_local = tid / G::L;
+    const unsigned hel = tid % G::L;
+    const int64_t ev0 = (int64_t)blockIdx.x * G::EPB;
+    {
+        const double2* src = reinterpret_cast<const double2*>(momenta);
+        double2* dst = reinterpret_cast<double2*>(s_mom);
+        for (int idx = tid; idx < G::EPB * MOM / 2; idx += G::THREADS) {
+            int64_t e = ev0 + idx / (MOM / 2);
+            if (e >= n_events) e = n_events - 1;
+            dst[idx] = src[e * (MOM / 2) + idx % (MOM / 2)];
+        }
+    }
+    __syncthreads();
+
+    const double* mom = s_mom + ev_local * MOM;
+    const double shat = 4.0 * mom[0] * mom[4];  // (p1+p2)^2 for p1 || +z, p2 || -z
+    const double scale = (sizeof(T) == 4) ? sqrt(shat) : 1.0;
+    if (hel < (unsigned)N)
+        s_s2[ev_local * N + hel] = make_photon_entries<T>(mom + 4 * (2 + hel), &s_E[(ev_local * N + hel) * 2 + 1],
+                                                          &s_E[(ev_local * N + hel) * 2 + 0]);
+    if (hel >= 1u && hel <= (unsigned)(G::L - 2)) {
+        if constexpr (sizeof(T) == 4)
+            make_subset_entry_plain<N>(mom, hel, g, scale, &s_P[ev_local * G::L + hel]);
+        else
+            make_subset_entry<N, T>(mom, hel, g, scale, &s_P[ev_local * G::L + hel]);
+    }
+    __syncthreads();
+}
+
+// a8: |ampsum|^2 summed over the event's 2^N lanes (warp shuffles, one shared-memory pass for
+// N > 5), times the constant factors, one store per event.
+template <int N, typename T>
+__device__ __forceinline__ void finish_event(T ar, T ai, const double* s_mom, const double* s_s2, double* s_red,
+                                             double g, double* __restrict__ out, int64_t n_events)
+{
+    using G = Geometry<N>;
+    constexpr int MOM = 4 * (N + 2);
+    const int tid = threadIdx.x;
+    const int ev_local = tid / G::L;
+    const unsigned hel = tid % G::L;
+    const int64_t ev0 = (int64_t)blockIdx.x * G::EPB;
+    double m2 = (double)ar * (double)ar + (double)ai * (double)ai;
+    constexpr int WL = (G::L < 32) ? G::L : 32;
+#pragma unroll
+    for (int off = WL / 2; off > 0; off >>= 1) m2 += __shfl_xor_sync(0xffffffffu, m2, off);
+    if constexpr (G::L > 32) {
+        if ((tid & 31) == 0) s_red[tid >> 5] = m2;
+        __syncthreads();
+        if (hel == 0) {
+            m2 = 0.0;
+#pragma unroll
+            for (int w = 0; w < G::L / 32; ++w) m2 += s_red[ev_local * (G::L / 32) + w];
+        }
+    }
+    if (hel == 0 && ev0 + ev_local < n_events) {
+        // constants: 2 (parity) * g^2 (closing vertex) * 2E1*2E2 = s_hat (spinor norms) * 2^-N
+        // (the sqrt(2) of every polarisation vector) * prod s_i^2 (E' normalisation);
+        // fp32 worked in units of sqrt(s_hat)
+        const double* mom = s_mom + ev_local * MOM;
+        const double shat = 4.0 * mom[0] * mom[4];
+        double f = 2.0 * g * g * shat;
+#pragma unroll
+        for (int i = 0; i < N; ++i) f *= 0.5 * s_s2[ev_local * N + i];
+        if (sizeof(T) == 4) {
+            const double inv = 1.0 / shat;
+#pragma unroll
+            for (int i = 0; i < N - 1; ++i) f *= inv;
+        }
+        out[ev0 + ev_local] = f * m2;
+    }
+}

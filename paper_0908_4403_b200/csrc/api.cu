@@ -68,7 +68,14 @@ int heget_init(int device, double alpha, double q_charge, double pt_cut, double 
     }
     if (err == cudaSuccess) err = cudaMalloc(&ctx->d_stage_out3, sizeof(double) * 3);
     if (err == cudaSuccess) err = cudaStreamCreateWithFlags(&ctx->host_stream, cudaStreamNonBlocking);
+    if (err == cudaSuccess) err = cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking);
+    for (int c = 0; c < kHostChunks && err == cudaSuccess; ++c)
+        err = cudaEventCreateWithFlags(&ctx->chunk_ready[c], cudaEventDisableTiming);
     if (err != cudaSuccess) {
+        for (int c = 0; c < kHostChunks; ++c)
+            if (ctx->chunk_ready[c]) cudaEventDestroy(ctx->chunk_ready[c]);
+        if (ctx->host_stream) cudaStreamDestroy(ctx->host_stream);
+        if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
         cudaFree(ctx->d_partials);
         cudaFree(ctx->d_stage_out3);
         delete ctx;
@@ -85,7 +92,10 @@ void heget_destroy(heget_ctx* ctx)
     free_staging(ctx);
     cudaFree(ctx->d_partials);
     cudaFree(ctx->d_stage_out3);
+    for (int c = 0; c < kHostChunks; ++c)
+        if (ctx->chunk_ready[c]) cudaEventDestroy(ctx->chunk_ready[c]);
     if (ctx->host_stream) cudaStreamDestroy(ctx->host_stream);
+    if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
     delete ctx;
 }
 
@@ -131,13 +141,22 @@ int heget_rambo(heget_ctx* ctx, uint64_t seed, int n, double sqrt_s_hat, int64_t
 
 int heget_amp2(heget_ctx* ctx, const double* momenta, int n, int precision, double* out_amp2, int64_t N, void* stream)
 {
+    return heget_amp2_algo(ctx, momenta, n, precision, HEGET_ALGO_TREE, out_amp2, N, stream);
+}
+
+int heget_amp2_algo(heget_ctx* ctx, const double* momenta, int n, int precision, int algo, double* out_amp2,
+                    int64_t N, void* stream)
+{
+    if (algo != HEGET_ALGO_TREE && algo != HEGET_ALGO_SUBSET) return HEGET_EINVAL;
     if (!ctx || n < 2 || n > 8 || N < 0 || (N > 0 && (!momenta || !out_amp2))) return HEGET_EINVAL;
     if (precision != HEGET_FP32 && precision != HEGET_FP64) return HEGET_EINVAL;
     if ((reinterpret_cast<uintptr_t>(momenta) & 15u) != 0) return HEGET_EINVAL;
     DeviceGuard guard(ctx->device);
     if (!guard.ok) return fail_cuda(ctx, cudaGetLastError());
     int launches = 0;
-    cudaError_t err = heget_launch_amp2(ctx, momenta, n, precision, out_amp2, N, (cudaStream_t)stream, &launches);
+    cudaError_t err = (algo == HEGET_ALGO_SUBSET)
+                          ? heget_launch_amp2_subset(ctx, momenta, n, precision, out_amp2, N, (cudaStream_t)stream, &launches)
+                          : heget_launch_amp2(ctx, momenta, n, precision, out_amp2, N, (cudaStream_t)stream, &launches);
     ctx->launches += launches;
     return err == cudaSuccess ? HEGET_OK : fail_cuda(ctx, err);
 }
@@ -177,14 +196,28 @@ int heget_xsec_host(heget_ctx* ctx, const double* momenta, const double* weight,
         ctx->stage_events = cap_n * 10;
         ctx->stage_n_events = cap_n;
     }
-    cudaStream_t st = ctx->host_stream;
+    cudaStream_t st = ctx->host_stream, cp = ctx->copy_stream;
     int launches = 0, l2 = 0;
     if (N > 0) {
-        err = cudaMemcpyAsync(ctx->d_stage_mom, momenta, sizeof(double) * 4 * need, cudaMemcpyHostToDevice, st);
-        if (err == cudaSuccess)
-            err = cudaMemcpyAsync(ctx->d_stage_w, weight, sizeof(double) * N, cudaMemcpyHostToDevice, st);
-        if (err == cudaSuccess)
-            err = heget_launch_amp2(ctx, ctx->d_stage_mom, n, precision, ctx->d_stage_amp2, N, st, &launches);
+        // H2D of chunk c+1 overlaps the amplitude kernel of chunk c (two streams, one event
+        // per chunk); per-event results do not depend on how a batch is cut into launches
+        const int chunks = (N >= 64 * 1024) ? kHostChunks : 1;
+        const int64_t per = (N + chunks - 1) / chunks;
+        const size_t ev_bytes = sizeof(double) * 4 * (size_t)(n + 2);
+        err = cudaMemcpyAsync(ctx->d_stage_w, weight, sizeof(double) * N, cudaMemcpyHostToDevice, cp);
+        for (int c = 0; c < chunks && err == cudaSuccess; ++c) {
+            const int64_t lo = c * per, cnt = (lo + per <= N) ? per : N - lo;
+            if (cnt <= 0) break;
+            err = cudaMemcpyAsync(ctx->d_stage_mom + lo * 4 * (n + 2), momenta + lo * 4 * (n + 2), ev_bytes * cnt,
+                                  cudaMemcpyHostToDevice, cp);
+            if (err == cudaSuccess) err = cudaEventRecord(ctx->chunk_ready[c], cp);
+            if (err == cudaSuccess) err = cudaStreamWaitEvent(st, ctx->chunk_ready[c], 0);
+            int l1 = 0;
+            if (err == cudaSuccess)
+                err = heget_launch_amp2(ctx, ctx->d_stage_mom + lo * 4 * (n + 2), n, precision,
+                                        ctx->d_stage_amp2 + lo, cnt, st, &l1);
+            launches += l1;
+        }
     }
     if (err == cudaSuccess) err = heget_launch_reduce(ctx, ctx->d_stage_amp2, ctx->d_stage_w, n, N, ctx->d_stage_out3, st, &l2);
     ctx->launches += launches + l2;

@@ -6,6 +6,8 @@
 
 #include "../../include/heget.h"
 
+constexpr int kHostChunks = 8;  // pipeline depth of heget_xsec_host
+
 struct heget_ctx {
     int device;
     int sm_count;
@@ -20,7 +22,9 @@ struct heget_ctx {
     double* d_stage_out3;
     int64_t stage_events;   // capacity of the staging buffers, in events * (n+2)
     int64_t stage_n_events;
-    cudaStream_t host_stream;
+    cudaStream_t host_stream;   // compute stream of the *_host entry point
+    cudaStream_t copy_stream;   // its H2D stream: chunk c+1 is copied while chunk c is computed
+    cudaEvent_t chunk_ready[kHostChunks];
     int64_t launches;
     char cuda_msg[256];
 };
@@ -30,6 +34,8 @@ constexpr int kReduceBlocks = 296;  // 2 CTAs per SM on a 148-SM B200; any value
 // launchers (each returns a cudaError_t from the launch)
 cudaError_t heget_launch_amp2(const heget_ctx* ctx, const double* momenta, int n, int precision,
                               double* out_amp2, int64_t N, cudaStream_t stream, int* launches);
+cudaError_t heget_launch_amp2_subset(const heget_ctx* ctx, const double* momenta, int n, int precision,
+                                     double* out_amp2, int64_t N, cudaStream_t stream, int* launches);
 cudaError_t heget_launch_gen(const heget_ctx* ctx, uint64_t seed, int n, const heget_gen_cfg* cfg,
                              uint64_t first_event, int64_t N, double* momenta, double* weight,
                              cudaStream_t stream, int* launches);

@@ -13,7 +13,7 @@ import pytest
 import torch
 
 import oracle
-from paper_0908_4403_b200 import FP32, FP64, Heget, workloads
+from paper_0908_4403_b200 import ALGO_SUBSET, ALGO_TREE, FP32, FP64, Heget, workloads
 
 pytestmark = pytest.mark.gpu
 
@@ -45,9 +45,13 @@ def oracle_amp2_cached(key, mom, extended):
     return _ORACLE_CACHE[key]
 
 
-def gpu_amp2(hg, mom, precision):
+ALGOS = [ALGO_TREE, ALGO_SUBSET]
+ALGO_NAME = {ALGO_TREE: "tree", ALGO_SUBSET: "subset"}
+
+
+def gpu_amp2(hg, mom, precision, algo=ALGO_TREE):
     d = torch.from_numpy(mom).cuda()
-    out = hg.amp2(d, precision)
+    out = hg.amp2(d, precision, algo=algo)
     torch.cuda.synchronize()
     return out.cpu().numpy()
 
@@ -66,7 +70,8 @@ if HEAVY:
 
 @pytest.mark.parametrize("name", workloads.ORDER)
 @pytest.mark.parametrize("precision", [FP64, FP32])
-def test_amp2_matches_oracle_on_config_events(hg, name, precision):
+@pytest.mark.parametrize("algo", ALGOS)
+def test_amp2_matches_oracle_on_config_events(hg, name, precision, algo):
     n = workloads.CONFIGS[name]["n"]
     N = SMALL[name]
     mom, w = oracle_events(name, N)
@@ -76,11 +81,11 @@ def test_amp2_matches_oracle_on_config_events(hg, name, precision):
         idx = np.concatenate([np.flatnonzero(wb != 0)[: N - 1], np.flatnonzero(wb == 0)[:1]])
         mom, w = big[idx], wb[idx]
     ref = oracle_amp2_cached(name, mom, extended=(n <= 7 or HEAVY))
-    got = gpu_amp2(hg, mom, precision)
+    got = gpu_amp2(hg, mom, precision, algo)
     assert got.shape == ref.shape and np.all(np.isfinite(got)) and np.all(got > 0)
     rel = np.abs(got / ref - 1.0)
     passing = (w != 0) if workloads.CONFIGS[name]["apply_cuts"] else np.ones(len(w), bool)
-    report("%s %s" % (name, "fp64" if precision == FP64 else "fp32"), rel, passing)
+    report("%s %s %s" % (name, "fp64" if precision == FP64 else "fp32", ALGO_NAME[algo]), rel, passing)
     tol = TOL64 if precision == FP64 else TOL32
     assert passing.sum() >= 1
     assert np.all(rel[passing] <= tol)
@@ -89,56 +94,60 @@ def test_amp2_matches_oracle_on_config_events(hg, name, precision):
 
 @pytest.mark.parametrize("n", [3, 5])
 @pytest.mark.parametrize("precision", [FP64, FP32])
-def test_amp2_matches_oracle_other_multiplicities(hg, n, precision):
+@pytest.mark.parametrize("algo", ALGOS)
+def test_amp2_matches_oracle_other_multiplicities(hg, n, precision, algo):
     N = {3: 32 * 4 + 7, 5: 8 * 5 + 3}[n]
     mom, w = oracle.gen_events(5, n, N, mode=oracle.MODE_LOGUNIFORM, a=300.0, b=4000.0, y_max=1.5,
                                apply_cuts=True)
     ref = oracle_amp2_cached("other%d" % n, mom, extended=True)
-    got = gpu_amp2(hg, mom, precision)
+    got = gpu_amp2(hg, mom, precision, algo)
     rel = np.abs(got / ref - 1.0)
-    report("n=%d %s" % (n, "fp64" if precision == FP64 else "fp32"), rel, w != 0)
+    report("n=%d %s %s" % (n, "fp64" if precision == FP64 else "fp32", ALGO_NAME[algo]), rel, w != 0)
     tol = TOL64 if precision == FP64 else TOL32
     assert np.all(rel[w != 0] <= tol) and np.all(rel <= tol * 1e3)
 
 
-def test_amp2_two_photon_closed_form_fixed_energy(hg):
+@pytest.mark.parametrize("algo", ALGOS)
+def test_amp2_two_photon_closed_form_fixed_energy(hg, algo):
     # config 1 as specified: 65,536 events, fixed 1 TeV, no cuts -- all events bind
     mom, _ = oracle_events("2gamma", 1 << 16)
-    ref = oracle.amp2(mom, extended=True)
-    got = gpu_amp2(hg, mom, FP64)
+    ref = oracle_amp2_cached("2gamma_full", mom, extended=True)
+    got = gpu_amp2(hg, mom, FP64, algo)
     rel = np.abs(got / ref - 1.0)
     report("2gamma full fp64", rel, np.ones(len(rel), bool))
     assert np.all(rel <= TOL64)
-    got32 = gpu_amp2(hg, mom, FP32)
+    got32 = gpu_amp2(hg, mom, FP32, algo)
     rel32 = np.abs(got32 / ref - 1.0)
     report("2gamma full fp32", rel32, np.ones(len(rel), bool))
     assert np.all(rel32 <= TOL32)
 
 
 @pytest.mark.parametrize("n", [2, 4, 7])
-def test_amp2_edge_sizes(hg, n):
+@pytest.mark.parametrize("algo", ALGOS)
+def test_amp2_edge_sizes(hg, n, algo):
     mom, _ = oracle.gen_events(9, n, 3, mode=oracle.MODE_FIXED, a=800.0)
     ref = oracle.amp2(mom)
     # N = 0: nothing written, no error
     empty = torch.empty((0, n + 2, 4), dtype=torch.float64, device="cuda")
-    assert hg.amp2(empty).shape == (0,)
+    assert hg.amp2(empty, algo=algo).shape == (0,)
     # N = 1 and a sub-CTA batch
     for N in (1, 3):
-        got = gpu_amp2(hg, mom[:N], FP64)
+        got = gpu_amp2(hg, mom[:N], FP64, algo)
         assert np.all(np.abs(got / ref[:N] - 1.0) < 1e-11)
     # the output buffer is written only inside [0, N)
     out = torch.full((5,), -7.0, dtype=torch.float64, device="cuda")
-    hg.amp2(torch.from_numpy(mom).cuda(), FP64, out=out[:3])
+    hg.amp2(torch.from_numpy(mom).cuda(), FP64, out=out[:3], algo=algo)
     torch.cuda.synchronize()
     assert out[3].item() == -7.0 and out[4].item() == -7.0
 
 
-def test_amp2_is_deterministic_and_batch_independent(hg):
+@pytest.mark.parametrize("algo", ALGOS)
+def test_amp2_is_deterministic_and_batch_independent(hg, algo):
     mom, _ = oracle_events("4gamma", 1000)
-    a = gpu_amp2(hg, mom, FP64)
-    b = gpu_amp2(hg, mom, FP64)
+    a = gpu_amp2(hg, mom, FP64, algo)
+    b = gpu_amp2(hg, mom, FP64, algo)
     assert np.array_equal(a, b)
-    c = gpu_amp2(hg, mom[123:777], FP64)     # different CTA alignment, same per-event result
+    c = gpu_amp2(hg, mom[123:777], FP64, algo)     # different CTA alignment, same per-event result
     assert np.array_equal(a[123:777], c)
 
 
@@ -154,5 +163,7 @@ def test_invalid_arguments_return_einval(hg):
     assert lib.heget_amp2(ctx, None, 4, FP64, out.data_ptr(), 4, None) == -1
     assert lib.heget_amp2(ctx, buf.data_ptr() + 8, 4, FP64, out.data_ptr(), 1, None) == -1   # misaligned
     assert lib.heget_amp2(None, buf.data_ptr(), 4, FP64, out.data_ptr(), 4, None) == -1
+    assert lib.heget_amp2_algo(ctx, buf.data_ptr(), 4, FP64, 2, out.data_ptr(), 4, None) == -1       # unknown algo
+    assert lib.heget_amp2_algo(ctx, buf.data_ptr(), 4, FP64, ALGO_SUBSET, out.data_ptr(), 4, None) == 0
     assert lib.heget_xsec_reduce(ctx, out.data_ptr(), out.data_ptr(), 4, 4, None, None) == -1
     assert b"invalid" in lib.heget_strerror(-1)
