@@ -133,7 +133,7 @@ def run_reference(args):
         "gpu_launches": 0}))
 
 
-def time_config(hg, torch, name, precision, steps, warmup, flush, first_event, n_local):
+def time_config(hg, torch, name, precision, steps, warmup, flush, first_event, n_local, algo=0):
     """Device-timed steps of amp2 + xsec_reduce on resident inputs.  Returns per-step ms (whole
     step) and the amp2 kernel's own ms, both from CUDA events on the launching stream."""
     from paper_0908_4403_b200 import FP32, FP64, workloads
@@ -147,7 +147,7 @@ def time_config(hg, torch, name, precision, steps, warmup, flush, first_event, n
     def step(ev=None):
         if ev:
             ev[0].record()
-        hg.amp2(mom, prec, out=amp2)
+        hg.amp2(mom, prec, out=amp2, algo=algo)
         if ev:
             ev[1].record()
         hg.xsec_reduce(amp2, w, cfg["n"], out3=out3)
@@ -203,10 +203,10 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    def timed_run(name, precision, steps, warmup):
+    def timed_run(name, precision, steps, warmup, algo=0):
         c = workloads.CONFIGS[name]
         nl = c["N"]
-        mom, w, out3, step, evs, _ = time_config(hg, torch, name, precision, steps, warmup, None, rank * nl, nl)
+        mom, w, out3, step, evs, _ = time_config(hg, torch, name, precision, steps, warmup, None, rank * nl, nl, algo)
         barrier()
         for ev in evs:
             flush_buf.zero_()                                  # L2 flush, outside the timed events
@@ -313,7 +313,11 @@ def main():
                 nph = workloads.CONFIGS[name]["n"]
                 pk = peak_measured if precision == args.precision else hg.fma_peak(FP64 if precision == "fp64" else FP32)
                 ach = executed_flops_per_event(nph) * nn / (a_ms * 1e-3)
-                table.append({"workload": name, "n": nph, "precision": precision, "events": nn,
+                _, s_ms, _, _, _ = timed_run(name, precision, 3, 3, algo=1)
+                table.append({"workload": name, "n": nph, "precision": precision, "events": nn, "algo": "subset",
+                              "amp2_ms": s_ms, "events_per_s": nn / (s_ms * 1e-3),
+                              "note": "HEGET_ALGO_SUBSET (heget_amp2_algo): not the permutation tree, own flop count"})
+                table.append({"workload": name, "n": nph, "precision": precision, "events": nn, "algo": "tree",
                               "amp2_ms": a_ms, "events_per_s": nn / (a_ms * 1e-3),
                               "executed_tflops": ach / 1e12, "frac_of_measured_peak": ach / pk,
                               "model_c_tflops": model_flops_per_event(nph) * nn / (a_ms * 1e-3) / 1e12})

@@ -11,6 +11,8 @@ Functions (all citations are PAPER.md lines, see the C sources):
   gen_events(...)                                  Philox + RAMBO + boost + cuts + weight
   xsec_reduce(amp2, weight, n)                     step 6 sums
   philox4x32_10(ctr, key), uniforms(seed, event, slot), phase_space_volume(n, s)
+  helicity_bits(seed, event, n), amp2_sampled(seed, momenta, ...)   one random helicity per event
+  histogram(momenta, value, observable, lo, hi, nbins)              Fig. 2 distributions
 """
 import ctypes
 import os
@@ -20,7 +22,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libheget_oracle.so")
-_SOURCES = ["heget_oracle.c", "heget_oracle_gen.c"]
+_SOURCES = ["heget_oracle.c", "heget_oracle_gen.c", "heget_oracle_next1.c"]
 _DEPS = _SOURCES + ["amp_body.inc"]
 _lib = None
 
@@ -78,6 +80,14 @@ def _load():
     lib.heget_oracle_gamma.restype = None
     lib.heget_oracle_wavefunction.argtypes = [ctypes.c_int, dp, ctypes.c_int, ctypes.c_int, dp]
     lib.heget_oracle_wavefunction.restype = None
+    lib.heget_oracle_helicity_bits.argtypes = [ctypes.c_uint64, ctypes.c_uint64, ctypes.c_int]
+    lib.heget_oracle_helicity_bits.restype = ctypes.c_uint32
+    lib.heget_oracle_amp2_sampled.argtypes = [ctypes.c_uint64, ctypes.c_uint64, dp, ctypes.c_int, ctypes.c_int64,
+                                              ctypes.c_double, ctypes.c_int, dp, ctypes.POINTER(ctypes.c_int32)]
+    lib.heget_oracle_amp2_sampled.restype = None
+    lib.heget_oracle_histogram.argtypes = [dp, dp, ctypes.c_int, ctypes.c_int64, ctypes.c_int, ctypes.c_double,
+                                           ctypes.c_double, ctypes.c_int, dp]
+    lib.heget_oracle_histogram.restype = None
     _lib = lib
     return lib
 
@@ -183,3 +193,38 @@ def xsec_reduce(amp2_values, weight, n):
     out = np.zeros(3, dtype=np.float64)
     lib.heget_oracle_xsec_reduce(_dptr(a), _dptr(w), a.shape[0], int(n), _dptr(out))
     return out
+
+
+OBS_PT_MAX, OBS_DR_MIN, OBS_DR_ALL = 0, 1, 2
+
+
+def helicity_bits(seed, event, n):
+    """The n+2 helicity bits of one event (bit b: particle b, 1 -> +1); R21."""
+    return int(_load().heget_oracle_helicity_bits(int(seed), int(event), int(n)))
+
+
+def amp2_sampled(seed, momenta, g=G_DEFAULT, first_event=0, extended=False):
+    """4 * 2^n * |M(h_e)|^2 with one Philox-drawn helicity assignment per event -> (values[N], bits[N])."""
+    lib = _load()
+    momenta = np.ascontiguousarray(momenta, dtype=np.float64)
+    N, n = momenta.shape[0], momenta.shape[1] - 2
+    out = np.zeros(N, dtype=np.float64)
+    hel = np.zeros(N, dtype=np.int32)
+    if N > 0:
+        lib.heget_oracle_amp2_sampled(int(seed), int(first_event), _dptr(momenta), n, N, float(g),
+                                      int(bool(extended)), _dptr(out),
+                                      hel.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)))
+    return out, hel
+
+
+def histogram(momenta, value, observable, lo, hi, nbins):
+    """Weighted histogram [underflow, bins..., overflow] of max pT / min Delta R / all Delta R."""
+    lib = _load()
+    momenta = np.ascontiguousarray(momenta, dtype=np.float64)
+    value = np.ascontiguousarray(value, dtype=np.float64)
+    N, n = momenta.shape[0], momenta.shape[1] - 2
+    assert value.shape == (N,)
+    hist = np.zeros(nbins + 2, dtype=np.float64)
+    lib.heget_oracle_histogram(_dptr(momenta), _dptr(value), n, N, int(observable), float(lo), float(hi),
+                               int(nbins), _dptr(hist))
+    return hist
