@@ -113,6 +113,34 @@ enum { HEGET_ALGO_TREE = 0, HEGET_ALGO_SUBSET = 1 };
 int heget_amp2_algo(heget_ctx* ctx, const double* momenta, int n, int precision, int algo,
                     double* out_amp2, int64_t N, void* stream);
 
+/* The paper's own event loop (step 4 of PAPER.md:116-122): ONE random helicity assignment per
+ * event instead of the explicit helicity sum.  Event e (global index first_event + e) draws
+ * Philox4x32-10 with key `seed` and counter (event_lo, event_hi, 15, 0); bit b of the first
+ * output word is the helicity of particle b in the order u, ubar, gamma_1..gamma_n (1 -> +1,
+ * 0 -> -1).  out_amp2[e] = 4 * 2^n * |M(h_e)|^2, whose mean over h is the helicity sum that
+ * heget_amp2 returns (exactly 0 for sigma_1 = sigma_2); out_hel[e] = the n+2 bits drawn
+ * (step 5), or pass NULL.  Permutation tree as heget_amp2, one warp per event.
+ *   momenta [dev] const double[N][n+2][4]; out_amp2 [dev] double[N]; out_hel [dev] int32[N]. */
+int heget_amp2_sampled(heget_ctx* ctx, uint64_t seed, uint64_t first_event, const double* momenta,
+                       int n, int precision, double* out_amp2, int32_t* out_hel, int64_t N,
+                       void* stream);
+
+/* Kinematical distributions of Fig. 2 as weighted histograms, filled on the
+ * device: event e adds value[e] (e.g. weight * amp2; 0 = event failed the cuts, skipped) at
+ *   HEGET_OBS_PT_MAX  max_i pT(gamma_i)                         (eq. 9)
+ *   HEGET_OBS_DR_MIN  min_{i<j} Delta R_ij                      (eq. 10)
+ *   HEGET_OBS_DR_ALL  every Delta R_ij (n(n-1)/2 entries per event)
+ * with eta = asinh(pz/pT) and Delta phi wrapped to [0, pi].  nbins equal bins on [lo, hi):
+ * hist[0] = underflow (x < lo), hist[1..nbins], hist[nbins+1] = overflow (x >= hi or NaN).
+ * hist is zeroed by the call.  1 <= nbins <= HEGET_HIST_MAX_BINS, hi > lo, else HEGET_EINVAL.
+ * Additions are fp64 atomics: bin assignment is deterministic, the summation order is not.
+ *   momenta [dev] const double[N][n+2][4]; value [dev] const double[N];
+ *   hist [dev] double[nbins+2], written. */
+enum { HEGET_OBS_PT_MAX = 0, HEGET_OBS_DR_MIN = 1, HEGET_OBS_DR_ALL = 2 };
+#define HEGET_HIST_MAX_BINS 4094
+int heget_histogram(heget_ctx* ctx, const double* momenta, const double* value, int n, int64_t N,
+                    int observable, double lo, double hi, int nbins, double* hist, void* stream);
+
 /* Step 6 of PAPER.md:141 on the device: with x_e = weight[e] * amp2[e] * (1/4)(1/9)(1/n!)
  * (helicity average, colour factor and identical-photon factor of eq. 2, PAPER.md:37;
  * DESIGN.md R1 for the colour factor),

@@ -13,10 +13,11 @@ LIB_PATH = os.path.join(_HERE, "libheget.so")
 
 FP32, FP64 = 0, 1
 ALGO_TREE, ALGO_SUBSET = 0, 1
+OBS_PT_MAX, OBS_DR_MIN, OBS_DR_ALL = 0, 1, 2
 GEN_FIXED, GEN_LOGUNIFORM, GEN_TOYPDF = 0, 1, 2
 
 EXPORTS = ["heget_init", "heget_destroy", "heget_strerror", "heget_last_cuda_error", "heget_rambo",
-           "heget_gen_events", "heget_amp2", "heget_amp2_algo", "heget_xsec_reduce", "heget_xsec_host", "heget_fma_peak", "heget_fma_peak_pattern",
+           "heget_gen_events", "heget_amp2", "heget_amp2_algo", "heget_amp2_sampled", "heget_histogram", "heget_xsec_reduce", "heget_xsec_host", "heget_fma_peak", "heget_fma_peak_pattern",
            "heget_launch_count"]
 
 
@@ -59,6 +60,10 @@ def load_library():
     lib.heget_amp2.restype = ci
     lib.heget_amp2_algo.argtypes = [vp, dp, ci, ci, ci, dp, i64, vp]
     lib.heget_amp2_algo.restype = ci
+    lib.heget_amp2_sampled.argtypes = [vp, u64, u64, dp, ci, ci, dp, vp, i64, vp]
+    lib.heget_amp2_sampled.restype = ci
+    lib.heget_histogram.argtypes = [vp, dp, dp, ci, i64, ci, cd, cd, ci, dp, vp]
+    lib.heget_histogram.restype = ci
     lib.heget_xsec_reduce.argtypes = [vp, dp, dp, ci, i64, dp, vp]
     lib.heget_xsec_reduce.restype = ci
     lib.heget_xsec_host.argtypes = [vp, dp, dp, ci, ci, i64, dp, dp]
@@ -143,6 +148,35 @@ class Heget:
         self._check(self._lib.heget_amp2_algo(self._ctx, momenta.data_ptr(), n, precision, algo, out.data_ptr(), N,
                                               _stream_ptr(self.device)), "heget_amp2_algo")
         return out
+
+    def amp2_sampled(self, seed, momenta, precision=FP64, first_event=0, out=None, out_hel=None):
+        """One Philox-drawn helicity assignment per event: (4 * 2^n * |M(h)|^2 [N], bits [N] int32)."""
+        _check_dev(momenta, None, self.device)
+        if momenta.dim() != 3 or momenta.shape[2] != 4:
+            raise HegetError("momenta must be [N][n+2][4]")
+        N, n = momenta.shape[0], momenta.shape[1] - 2
+        if out is None:
+            out = torch.empty((N,), dtype=torch.float64, device=self.device)
+        if out_hel is None:
+            out_hel = torch.empty((N,), dtype=torch.int32, device=self.device)
+        _check_dev(out, (N,), self.device)
+        self._check(self._lib.heget_amp2_sampled(self._ctx, seed, first_event, momenta.data_ptr(), n, precision,
+                                                 out.data_ptr(), out_hel.data_ptr(), N,
+                                                 _stream_ptr(self.device)), "heget_amp2_sampled")
+        return out, out_hel
+
+    def histogram(self, momenta, value, observable, lo, hi, nbins, hist=None):
+        """Weighted histogram [underflow, nbins bins, overflow] of max pT / min Delta R / all Delta R."""
+        _check_dev(momenta, None, self.device)
+        N, n = momenta.shape[0], momenta.shape[1] - 2
+        _check_dev(value, (N,), self.device)
+        if hist is None:
+            hist = torch.empty((nbins + 2,), dtype=torch.float64, device=self.device)
+        _check_dev(hist, (nbins + 2,), self.device)
+        self._check(self._lib.heget_histogram(self._ctx, momenta.data_ptr(), value.data_ptr(), n, N, observable,
+                                              lo, hi, nbins, hist.data_ptr(), _stream_ptr(self.device)),
+                    "heget_histogram")
+        return hist
 
     def xsec_reduce(self, amp2, weight, n, out3=None):
         _check_dev(amp2, None, self.device)

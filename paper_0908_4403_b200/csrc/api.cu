@@ -161,6 +161,37 @@ int heget_amp2_algo(heget_ctx* ctx, const double* momenta, int n, int precision,
     return err == cudaSuccess ? HEGET_OK : fail_cuda(ctx, err);
 }
 
+int heget_amp2_sampled(heget_ctx* ctx, uint64_t seed, uint64_t first_event, const double* momenta, int n,
+                       int precision, double* out_amp2, int32_t* out_hel, int64_t N, void* stream)
+{
+    if (!ctx || n < 2 || n > 8 || N < 0 || (N > 0 && (!momenta || !out_amp2))) return HEGET_EINVAL;
+    if (precision != HEGET_FP32 && precision != HEGET_FP64) return HEGET_EINVAL;
+    if ((reinterpret_cast<uintptr_t>(momenta) & 15u) != 0) return HEGET_EINVAL;
+    DeviceGuard guard(ctx->device);
+    if (!guard.ok) return fail_cuda(ctx, cudaGetLastError());
+    int launches = 0;
+    cudaError_t err = heget_launch_amp2_sampled(ctx, seed, first_event, momenta, n, precision, out_amp2, out_hel, N,
+                                                (cudaStream_t)stream, &launches);
+    ctx->launches += launches;
+    return err == cudaSuccess ? HEGET_OK : fail_cuda(ctx, err);
+}
+
+int heget_histogram(heget_ctx* ctx, const double* momenta, const double* value, int n, int64_t N, int observable,
+                    double lo, double hi, int nbins, double* hist, void* stream)
+{
+    if (!ctx || n < 2 || n > 8 || N < 0 || !hist || (N > 0 && (!momenta || !value))) return HEGET_EINVAL;
+    if (observable < HEGET_OBS_PT_MAX || observable > HEGET_OBS_DR_ALL) return HEGET_EINVAL;
+    if (nbins < 1 || nbins > HEGET_HIST_MAX_BINS || !(hi > lo)) return HEGET_EINVAL;
+    if ((reinterpret_cast<uintptr_t>(momenta) & 15u) != 0) return HEGET_EINVAL;
+    DeviceGuard guard(ctx->device);
+    if (!guard.ok) return fail_cuda(ctx, cudaGetLastError());
+    int launches = 0;
+    cudaError_t err = heget_launch_histogram(ctx, momenta, value, n, N, observable, lo, hi, nbins, hist,
+                                             (cudaStream_t)stream, &launches);
+    ctx->launches += launches;
+    return err == cudaSuccess ? HEGET_OK : fail_cuda(ctx, err);
+}
+
 int heget_xsec_reduce(heget_ctx* ctx, const double* amp2, const double* weight, int n, int64_t N, double* out3,
                       void* stream)
 {
