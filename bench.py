@@ -25,7 +25,7 @@ if ROOT not in sys.path:
 METRIC = "events/s of summed |M|^2 for u ubar->n gamma"
 # dram__bytes_read.sum + dram__bytes_write.sum of one amp2 launch at the config's full size, from
 # the `ncu --set full` captures summarised under profiles/ (n, precision) -> bytes
-NCU_DRAM_BYTES = {}
+NCU_DRAM_BYTES = {(4, "fp64"): 211446528, (4, "fp32"): 210010112, (8, "fp64"): 21157888, (8, "fp32"): 21101824}
 UNIT = "events/s"
 
 
