@@ -19,30 +19,51 @@ struct Geometry {
     static constexpr int EPB = THREADS / L;                // events per CTA
 };
 
-// a1: coalesced double2 load of the CTA's momenta (events past the end re-read the last
-// event); a4: vxxxx0 for both helicities of photon `hel` (lanes 0..N-1 of each event);
-// a5: subset kinematics, one subset per lane.  Ends with a CTA barrier.
+// a1: the CTA's momenta as double2 words, PF words per thread: global -> registers
+// (events past the end re-read the last event) and registers -> shared memory.  Split in two
+// so that a persistent CTA can have the next batch's loads in flight while it computes.
+template <int N>
+struct MomentaTile {
+    using G = Geometry<N>;
+    static constexpr int MOM = 4 * (N + 2);
+    static constexpr int WORDS = G::EPB * MOM / 2;
+    static constexpr int PF = (WORDS + G::THREADS - 1) / G::THREADS;
+
+    static __device__ __forceinline__ void load(const double* __restrict__ momenta, int64_t ev0, int64_t n_events,
+                                                double2 (&r)[PF])
+    {
+        const double2* src = reinterpret_cast<const double2*>(momenta);
+#pragma unroll
+        for (int k = 0; k < PF; ++k) {
+            const int idx = threadIdx.x + k * G::THREADS;
+            if (idx < WORDS) {
+                int64_t e = ev0 + idx / (MOM / 2);
+                if (e >= n_events) e = n_events - 1;
+                r[k] = src[e * (MOM / 2) + idx % (MOM / 2)];
+            }
+        }
+    }
+    static __device__ __forceinline__ void store(double* s_mom, const double2 (&r)[PF])
+    {
+        double2* dst = reinterpret_cast<double2*>(s_mom);
+#pragma unroll
+        for (int k = 0; k < PF; ++k) {
+            const int idx = threadIdx.x + k * G::THREADS;
+            if (idx < WORDS) dst[idx] = r[k];
+        }
+    }
+};
+
+// a4: vxxxx0 for both helicities of photon `hel` (lanes 0..N-1 of each event);
+// a5: subset kinematics, one subset per lane.  Reads s_mom (barrier before), ends with a barrier.
 template <int N, typename T>
-__device__ __forceinline__ void build_event_tables(const double* __restrict__ momenta, int64_t n_events, double g,
-                                                   double* s_mom, PEntry<T>* s_P, EEntry<T>* s_E, double* s_s2)
+__device__ __forceinline__ void build_tables(double g, const double* s_mom, PEntry<T>* s_P, EEntry<T>* s_E,
+                                             double* s_s2)
 {
     using G = Geometry<N>;
     constexpr int MOM = 4 * (N + 2);
-    const int tid = threadIdx.x;
-    const int ev_local = tid / G::L;
-    const unsigned hel = tid % G::L;
-    const int64_t ev0 = (int64_t)blockIdx.x * G::EPB;
-    {
-        const double2* src = reinterpret_cast<const double2*>(momenta);
-        double2* dst = reinterpret_cast<double2*>(s_mom);
-        for (int idx = tid; idx < G::EPB * MOM / 2; idx += G::THREADS) {
-            int64_t e = ev0 + idx / (MOM / 2);
-            if (e >= n_events) e = n_events - 1;
-            dst[idx] = src[e * (MOM / 2) + idx % (MOM / 2)];
-        }
-    }
-    __syncthreads();
-
+    const int ev_local = threadIdx.x / G::L;
+    const unsigned hel = threadIdx.x % G::L;
     const double* mom = s_mom + ev_local * MOM;
     const double shat = 4.0 * mom[0] * mom[4];  // (p1+p2)^2 for p1 || +z, p2 || -z
     const double scale = (sizeof(T) == 4) ? sqrt(shat) : 1.0;
@@ -58,18 +79,30 @@ __device__ __forceinline__ void build_event_tables(const double* __restrict__ mo
     __syncthreads();
 }
 
+// a1 + a4 + a5 for the batch of events starting at ev0 (one-shot form).
+template <int N, typename T>
+__device__ __forceinline__ void build_event_tables(const double* __restrict__ momenta, int64_t ev0, int64_t n_events,
+                                                   double g, double* s_mom, PEntry<T>* s_P, EEntry<T>* s_E,
+                                                   double* s_s2)
+{
+    double2 r[MomentaTile<N>::PF];
+    MomentaTile<N>::load(momenta, ev0, n_events, r);
+    MomentaTile<N>::store(s_mom, r);
+    __syncthreads();
+    build_tables<N, T>(g, s_mom, s_P, s_E, s_s2);
+}
+
 // a8: |ampsum|^2 summed over the event's 2^N lanes (warp shuffles, one shared-memory pass for
 // N > 5), times the constant factors, one store per event.
 template <int N, typename T>
 __device__ __forceinline__ void finish_event(T ar, T ai, const double* s_mom, const double* s_s2, double* s_red,
-                                             double g, double* __restrict__ out, int64_t n_events)
+                                             double g, double* __restrict__ out, int64_t ev0, int64_t n_events)
 {
     using G = Geometry<N>;
     constexpr int MOM = 4 * (N + 2);
     const int tid = threadIdx.x;
     const int ev_local = tid / G::L;
     const unsigned hel = tid % G::L;
-    const int64_t ev0 = (int64_t)blockIdx.x * G::EPB;
     double m2 = (double)ar * (double)ar + (double)ai * (double)ai;
     constexpr int WL = (G::L < 32) ? G::L : 32;
 #pragma unroll

@@ -175,7 +175,7 @@ amp2_subset_kernel(const double* __restrict__ momenta, double* __restrict__ out,
 
     for (int i = threadIdx.x; i < 256; i += G::THREADS) s_rank[i] = c_index.rank[i];
     for (int i = threadIdx.x; i < (N + 1) * 72; i += G::THREADS) s_list[i] = c_index.list[i / 72][i % 72];
-    build_event_tables<N, T>(momenta, n_events, g, s_mom, s_P, s_E, s_s2);  // ends with a barrier
+    build_event_tables<N, T>(momenta, (int64_t)blockIdx.x * G::EPB, n_events, g, s_mom, s_P, s_E, s_s2);  // ends with a barrier
 
     const PEntry<T>* P = s_P + ev_local * G::L;
     const EEntry<T>* E = s_E + ev_local * 2 * N;
@@ -195,7 +195,7 @@ amp2_subset_kernel(const double* __restrict__ momenta, double* __restrict__ out,
         ar += fma(e.ar, f.r0, fma(-e.ai, f.i0, f.r1));
         ai += fma(e.ar, f.i0, fma(e.ai, f.r0, f.i1));
     }
-    finish_event<N, T>(ar, ai, s_mom, s_s2, s_red, g, out, n_events);
+    finish_event<N, T>(ar, ai, s_mom, s_s2, s_red, g, out, (int64_t)blockIdx.x * G::EPB, n_events);
 }
 
 template <int N, typename T>

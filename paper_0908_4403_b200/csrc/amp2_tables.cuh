@@ -107,17 +107,23 @@ __device__ __forceinline__ void make_subset_entry(const double* mom, unsigned S,
     for (int i = 0; i < N; ++i) {
         if ((S >> i) & 1u) {
             const double* k = mom + 4 * (2 + i);
-            pe = dd_add_d(pe, -k[0]);
-            px = dd_add_d(px, -k[1]);
-            py = dd_add_d(py, -k[2]);
-            pz = dd_add_d(pz, -k[3]);
+            dd_acc(pe, -k[0]);
+            dd_acc(px, -k[1]);
+            dd_acc(py, -k[2]);
+            dd_acc(pz, -k[3]);
         }
     }
-    const dd pp = dd_add(pe, pz);
-    const dd pm = dd_add(pe, dd_neg(pz));
-    dd t = dd_mul(pp, pm);
-    t = dd_add(t, dd_neg(dd_mul(px, px)));
-    t = dd_add(t, dd_neg(dd_mul(py, py)));
+    // p+- = pe +- pz: high parts by TwoSum, low parts added
+    dd pp = dd_two_sum(pe.hi, pz.hi), pm = dd_two_sum(pe.hi, -pz.hi);
+    pp.lo = __dadd_rn(pp.lo, __dadd_rn(pe.lo, pz.lo));
+    pm.lo = __dadd_rn(pm.lo, __dsub_rn(pe.lo, pz.lo));
+    // t = p+ p- - px^2 - py^2: exact products of the high parts, first-order low parts
+    dd a = dd_two_prod(pp.hi, pm.hi), bx = dd_two_prod(px.hi, px.hi), by = dd_two_prod(py.hi, py.hi);
+    a.lo = __fma_rn(pp.hi, pm.lo, __fma_rn(pp.lo, pm.hi, a.lo));
+    bx.lo = __fma_rn(2.0 * px.hi, px.lo, bx.lo);
+    by.lo = __fma_rn(2.0 * py.hi, py.lo, by.lo);
+    const dd s1 = dd_two_sum(a.hi, -bx.hi), s2 = dd_two_sum(s1.hi, -by.hi);
+    const dd t = {s2.hi, __dadd_rn(__dadd_rn(s2.lo, s1.lo), __dsub_rn(__dsub_rn(a.lo, bx.lo), by.lo))};
     const double c = -g * scale * fast_rcp(dd_to_double(t));
     out->pp = (T)(c * dd_to_double(pp));
     out->pm = (T)(c * dd_to_double(pm));

@@ -32,6 +32,15 @@ __device__ __forceinline__ dd dd_two_prod(double a, double b)
     return {p, e};
 }
 
+// a += b without renormalising: the high part by TwoSum, its rounding error collected in the
+// low part (exact to ~2^-106 of the largest intermediate for the handful of terms summed here)
+__device__ __forceinline__ void dd_acc(dd& a, double b)
+{
+    const dd s = dd_two_sum(a.hi, b);
+    a.hi = s.hi;
+    a.lo = __dadd_rn(a.lo, s.lo);
+}
+
 __device__ __forceinline__ dd dd_add_d(dd a, double b)
 {
     dd s = dd_two_sum(a.hi, b);
