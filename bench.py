@@ -313,10 +313,13 @@ def main():
                 nph = workloads.CONFIGS[name]["n"]
                 pk = peak_measured if precision == args.precision else hg.fma_peak(FP64 if precision == "fp64" else FP32)
                 ach = executed_flops_per_event(nph) * nn / (a_ms * 1e-3)
-                _, s_ms, _, _, _ = timed_run(name, precision, 3, 3, algo=1)
-                table.append({"workload": name, "n": nph, "precision": precision, "events": nn, "algo": "subset",
-                              "amp2_ms": s_ms, "events_per_s": nn / (s_ms * 1e-3),
-                              "note": "HEGET_ALGO_SUBSET (heget_amp2_algo): not the permutation tree, own flop count"})
+                for algo_id, algo_name, note in (
+                        (1, "subset", "HEGET_ALGO_SUBSET (heget_amp2_algo): not the permutation tree, own flop count"),
+                        (2, "two-sided", "HEGET_ALGO_TREE2 (heget_amp2_algo): tree from u to depth n-3, closed with "
+                                         "row vectors chained from ubar; own flop count")):
+                    _, s_ms, _, _, _ = timed_run(name, precision, 3, 3, algo=algo_id)
+                    table.append({"workload": name, "n": nph, "precision": precision, "events": nn, "algo": algo_name,
+                                  "amp2_ms": s_ms, "events_per_s": nn / (s_ms * 1e-3), "note": note})
                 table.append({"workload": name, "n": nph, "precision": precision, "events": nn, "algo": "tree",
                               "amp2_ms": a_ms, "events_per_s": nn / (a_ms * 1e-3),
                               "executed_tflops": ach / 1e12, "frac_of_measured_peak": ach / pk,

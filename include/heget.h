@@ -108,8 +108,13 @@ int heget_amp2(heget_ctx* ctx, const double* momenta, int n, int precision, doub
  *                      collapse onto 2^n sets (3^n - 1 spinors per event including helicities).
  *                      Same result up to rounding order; NOT the permutation-tree method, hence a
  *                      separately named mode (reuse of off-shell lines).
+ *   HEGET_ALGO_TREE2   two-sided chaining: the permutation tree from the u end (fvixx0) is walked
+ *                      to depth n - min(n,3) only and every branch closes with one dot product
+ *                      against row vectors chained from the ubar end (fvoxx0 of List 2,
+ *                      PAPER.md:449-450, 642-656) and tabulated per photon set: the same n!
+ *                      diagrams with the off-shell lines near the ubar end shared.
  * Arguments, layout and errors as heget_amp2; algo outside the enum gives HEGET_EINVAL. */
-enum { HEGET_ALGO_TREE = 0, HEGET_ALGO_SUBSET = 1 };
+enum { HEGET_ALGO_TREE = 0, HEGET_ALGO_SUBSET = 1, HEGET_ALGO_TREE2 = 2 };
 int heget_amp2_algo(heget_ctx* ctx, const double* momenta, int n, int precision, int algo,
                     double* out_amp2, int64_t N, void* stream);
 

@@ -12,7 +12,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libheget.so")
 
 FP32, FP64 = 0, 1
-ALGO_TREE, ALGO_SUBSET = 0, 1
+ALGO_TREE, ALGO_SUBSET, ALGO_TREE2 = 0, 1, 2
 OBS_PT_MAX, OBS_DR_MIN, OBS_DR_ALL = 0, 1, 2
 GEN_FIXED, GEN_LOGUNIFORM, GEN_TOYPDF = 0, 1, 2
 

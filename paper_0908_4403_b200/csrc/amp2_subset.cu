@@ -20,41 +20,9 @@
 // C(N,m) 2^m items (S, helicities of S); levels are separated by CTA barriers and ping-pong
 // between two shared-memory buffers.
 #include "amp2_common.cuh"
+#include "subset_index.cuh"
 
 namespace {
-
-constexpr int kMaxN = 8;
-
-__host__ __device__ constexpr int binom(int n, int k)
-{
-    if (k < 0 || k > n) return 0;
-    int r = 1;
-    for (int i = 1; i <= k; ++i) r = r * (n - k + i) / i;
-    return r;
-}
-
-// rank[S]: position of S among the subsets with the same number of elements, in increasing
-// numeric order; list[m][r]: its inverse.  Independent of N for S < 2^N.
-struct SubsetIndex {
-    unsigned char rank[1 << kMaxN];
-    unsigned char list[kMaxN + 1][72];
-};
-
-constexpr SubsetIndex make_subset_index()
-{
-    SubsetIndex t{};
-    int count[kMaxN + 1] = {};
-    for (int S = 0; S < (1 << kMaxN); ++S) {
-        int m = 0;
-        for (int b = 0; b < kMaxN; ++b) m += (S >> b) & 1;
-        t.rank[S] = (unsigned char)count[m];
-        t.list[m][count[m]] = (unsigned char)S;
-        ++count[m];
-    }
-    return t;
-}
-
-__constant__ SubsetIndex c_index = make_subset_index();
 
 template <int N>
 __host__ __device__ constexpr int max_level_items()
@@ -173,8 +141,7 @@ amp2_subset_kernel(const double* __restrict__ momenta, double* __restrict__ out,
     const int ev_local = threadIdx.x / G::L;
     const unsigned hel = threadIdx.x % G::L;
 
-    for (int i = threadIdx.x; i < 256; i += G::THREADS) s_rank[i] = c_index.rank[i];
-    for (int i = threadIdx.x; i < (N + 1) * 72; i += G::THREADS) s_list[i] = c_index.list[i / 72][i % 72];
+    load_subset_index<N, G::THREADS>(s_rank, s_list);
     build_event_tables<N, T>(momenta, (int64_t)blockIdx.x * G::EPB, n_events, g, s_mom, s_P, s_E, s_s2);  // ends with a barrier
 
     const PEntry<T>* P = s_P + ev_local * G::L;

@@ -147,16 +147,20 @@ int heget_amp2(heget_ctx* ctx, const double* momenta, int n, int precision, doub
 int heget_amp2_algo(heget_ctx* ctx, const double* momenta, int n, int precision, int algo, double* out_amp2,
                     int64_t N, void* stream)
 {
-    if (algo != HEGET_ALGO_TREE && algo != HEGET_ALGO_SUBSET) return HEGET_EINVAL;
+    if (algo < HEGET_ALGO_TREE || algo > HEGET_ALGO_TREE2) return HEGET_EINVAL;
     if (!ctx || n < 2 || n > 8 || N < 0 || (N > 0 && (!momenta || !out_amp2))) return HEGET_EINVAL;
     if (precision != HEGET_FP32 && precision != HEGET_FP64) return HEGET_EINVAL;
     if ((reinterpret_cast<uintptr_t>(momenta) & 15u) != 0) return HEGET_EINVAL;
     DeviceGuard guard(ctx->device);
     if (!guard.ok) return fail_cuda(ctx, cudaGetLastError());
     int launches = 0;
-    cudaError_t err = (algo == HEGET_ALGO_SUBSET)
-                          ? heget_launch_amp2_subset(ctx, momenta, n, precision, out_amp2, N, (cudaStream_t)stream, &launches)
-                          : heget_launch_amp2(ctx, momenta, n, precision, out_amp2, N, (cudaStream_t)stream, &launches);
+    cudaError_t err;
+    if (algo == HEGET_ALGO_SUBSET)
+        err = heget_launch_amp2_subset(ctx, momenta, n, precision, out_amp2, N, (cudaStream_t)stream, &launches);
+    else if (algo == HEGET_ALGO_TREE2)
+        err = heget_launch_amp2_twosided(ctx, momenta, n, precision, out_amp2, N, (cudaStream_t)stream, &launches);
+    else
+        err = heget_launch_amp2(ctx, momenta, n, precision, out_amp2, N, (cudaStream_t)stream, &launches);
     ctx->launches += launches;
     return err == cudaSuccess ? HEGET_OK : fail_cuda(ctx, err);
 }

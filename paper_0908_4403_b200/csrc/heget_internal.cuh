@@ -36,6 +36,8 @@ cudaError_t heget_launch_amp2(const heget_ctx* ctx, const double* momenta, int n
                               double* out_amp2, int64_t N, cudaStream_t stream, int* launches);
 cudaError_t heget_launch_amp2_subset(const heget_ctx* ctx, const double* momenta, int n, int precision,
                                      double* out_amp2, int64_t N, cudaStream_t stream, int* launches);
+cudaError_t heget_launch_amp2_twosided(const heget_ctx* ctx, const double* momenta, int n, int precision,
+                                       double* out_amp2, int64_t N, cudaStream_t stream, int* launches);
 cudaError_t heget_launch_amp2_sampled(const heget_ctx* ctx, uint64_t seed, uint64_t first_event,
                                       const double* momenta, int n, int precision, double* out_amp2,
                                       int32_t* out_hel, int64_t N, cudaStream_t stream, int* launches);

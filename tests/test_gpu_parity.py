@@ -13,7 +13,7 @@ import pytest
 import torch
 
 import oracle
-from paper_0908_4403_b200 import ALGO_SUBSET, ALGO_TREE, FP32, FP64, Heget, workloads
+from paper_0908_4403_b200 import ALGO_SUBSET, ALGO_TREE, ALGO_TREE2, FP32, FP64, Heget, workloads
 
 pytestmark = pytest.mark.gpu
 
@@ -45,8 +45,8 @@ def oracle_amp2_cached(key, mom, extended):
     return _ORACLE_CACHE[key]
 
 
-ALGOS = [ALGO_TREE, ALGO_SUBSET]
-ALGO_NAME = {ALGO_TREE: "tree", ALGO_SUBSET: "subset"}
+ALGOS = [ALGO_TREE, ALGO_SUBSET, ALGO_TREE2]
+ALGO_NAME = {ALGO_TREE: "tree", ALGO_SUBSET: "subset", ALGO_TREE2: "two-sided"}
 
 
 def gpu_amp2(hg, mom, precision, algo=ALGO_TREE):
@@ -163,7 +163,7 @@ def test_invalid_arguments_return_einval(hg):
     assert lib.heget_amp2(ctx, None, 4, FP64, out.data_ptr(), 4, None) == -1
     assert lib.heget_amp2(ctx, buf.data_ptr() + 8, 4, FP64, out.data_ptr(), 1, None) == -1   # misaligned
     assert lib.heget_amp2(None, buf.data_ptr(), 4, FP64, out.data_ptr(), 4, None) == -1
-    assert lib.heget_amp2_algo(ctx, buf.data_ptr(), 4, FP64, 2, out.data_ptr(), 4, None) == -1       # unknown algo
+    assert lib.heget_amp2_algo(ctx, buf.data_ptr(), 4, FP64, 3, out.data_ptr(), 4, None) == -1       # unknown algo
     assert lib.heget_amp2_algo(ctx, buf.data_ptr(), 4, FP64, ALGO_SUBSET, out.data_ptr(), 4, None) == 0
     assert lib.heget_xsec_reduce(ctx, out.data_ptr(), out.data_ptr(), 4, 4, None, None) == -1
     assert b"invalid" in lib.heget_strerror(-1)

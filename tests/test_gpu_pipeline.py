@@ -8,7 +8,7 @@ import pytest
 import torch
 
 import oracle
-from paper_0908_4403_b200 import ALGO_SUBSET, FP32, FP64, Heget, workloads
+from paper_0908_4403_b200 import ALGO_SUBSET, ALGO_TREE2, FP32, FP64, Heget, workloads
 
 pytestmark = pytest.mark.gpu
 
@@ -165,14 +165,16 @@ def test_full_size_config_sampled_against_oracle(hg, name):
     lo = N // 2 + 1
     sub = hg.amp2(dm[lo:lo + 300].contiguous(), FP64).cpu().numpy()
     assert np.array_equal(sub, g64[lo:lo + 300])
-    # the subset-recursion mode (heget_amp2_algo, HEGET_ALGO_SUBSET) at the same full size:
-    # sampled events against the oracle, every passing event against the tree mode
-    s64 = hg.amp2(dm, FP64, algo=ALGO_SUBSET).cpu().numpy()
-    s32 = hg.amp2(dm, FP32, algo=ALGO_SUBSET).cpu().numpy()
-    q64 = np.abs(s64[idx] / ref - 1.0)
-    q32 = np.abs(s32[idx] / ref - 1.0)
-    print("[full-size parity] %s subset mode: fp64 max %.3e median %.3e; fp32 max %.3e median %.3e"
-          % (name, q64.max(), np.median(q64), q32.max(), np.median(q32)))
-    assert np.all(q64 <= 1e-12) and np.all(q32 <= 1e-4)
-    assert np.abs(s64[passing] / g64[passing] - 1.0).max() <= 2e-12
-    assert np.abs(s32[passing] / g64[passing] - 1.0).max() <= 1e-4
+    # the other organisations of the permutation sum (heget_amp2_algo: subset recursion,
+    # two-sided chaining) at the same full size: sampled events against the oracle, every
+    # passing event against the tree mode
+    for algo, tag in ((ALGO_SUBSET, "subset"), (ALGO_TREE2, "two-sided")):
+        s64 = hg.amp2(dm, FP64, algo=algo).cpu().numpy()
+        s32 = hg.amp2(dm, FP32, algo=algo).cpu().numpy()
+        q64 = np.abs(s64[idx] / ref - 1.0)
+        q32 = np.abs(s32[idx] / ref - 1.0)
+        print("[full-size parity] %s %s mode: fp64 max %.3e median %.3e; fp32 max %.3e median %.3e"
+              % (name, tag, q64.max(), np.median(q64), q32.max(), np.median(q32)))
+        assert np.all(q64 <= 1e-12) and np.all(q32 <= 1e-4)
+        assert np.abs(s64[passing] / g64[passing] - 1.0).max() <= 2e-12
+        assert np.abs(s32[passing] / g64[passing] - 1.0).max() <= 1e-4
