@@ -114,6 +114,54 @@ def test_xsec_host_equals_device_path(hg, precision):
     assert abs(out3[0].item() / ref[0] - 1.0) < tol and out3[2].item() == ref[2]
 
 
+def test_xsec_host_pipelined_chunks_equal_device_path(hg):
+    """N >= 65536 takes the chunked path (H2D of chunk c+1 overlapping chunk c's kernel); a ragged
+    N that the 8 chunks do not divide must give bit-identical amp2 and sums."""
+    N = 65536 + 4099
+    c = workloads.CONFIGS["2gamma"]
+    dm, dw = hg.gen_events(3, 2, N, mode=workloads.LOGUNIFORM, a=200.0, b=3000.0, y_max=1.5, apply_cuts=True)
+    hm, hw = dm.cpu().pin_memory(), dw.cpu().pin_memory()
+    out_amp2 = torch.empty(N, dtype=torch.float64).pin_memory()
+    for precision in (FP64, FP32):
+        out3 = hg.xsec_host(hm, hw, precision, out_amp2=out_amp2)
+        a = hg.amp2(dm, precision)
+        r = hg.xsec_reduce(a, dw, c["n"])
+        torch.cuda.synchronize()
+        assert torch.equal(a.cpu(), out_amp2) and torch.equal(r.cpu(), out3)
+        again = hg.xsec_host(hm, hw, precision)           # staging buffers reused
+        assert torch.equal(again, out3)
+
+
+def test_other_quark_flavour_rescales_with_charge(hg):
+    """SURVEY 8(f) NEXT-4, flavours: the amplitude is proportional to Q_q^n, so a d-type line
+    (Q = -1/3) gives (1/2)^(2n) of the u-type result; the oracle is evaluated with g of that
+    charge, the library through heget_init's q_charge."""
+    hd = Heget(0, workloads.ALPHA, -1.0 / 3.0, workloads.PT_CUT, workloads.ETA_CUT, workloads.DR_CUT)
+    try:
+        for n in (2, 5):
+            mom, w = oracle.gen_events(4, n, 40, mode=oracle.MODE_LOGUNIFORM, a=300.0, b=3000.0, y_max=1.5,
+                                       apply_cuts=True)
+            g_d = oracle.G_DEFAULT * (-1.0 / 3.0) / workloads.Q_U
+            ref = oracle.amp2(mom, g=g_d, extended=True)
+            d = torch.from_numpy(mom).cuda()
+            got_d = hd.amp2(d, FP64).cpu().numpy()
+            got_u = hg.amp2(d, FP64).cpu().numpy()
+            assert np.all(np.abs(got_d / ref - 1.0)[w != 0] <= 1e-12)
+            assert np.all(np.abs(got_d / got_u * 4.0 ** n - 1.0) <= 1e-13)
+    finally:
+        hd.close()
+
+
+def test_fma_peak_patterns_are_ordered(hg):
+    """Roofline denominators: constant-operand FMA >= node pattern >= three-register FMA, and the
+    constant-operand figure is within the B200's theoretical non-tensor peak."""
+    for prec, lanes in ((FP32, 128), (FP64, 64)):
+        p0, p1, p2 = (hg.fma_peak(prec, k) for k in (0, 1, 2))
+        sm = torch.cuda.get_device_properties(0).multi_processor_count
+        assert p0 <= sm * lanes * 2 * 2.2e9 and p0 >= 0.5 * sm * lanes * 2 * 1.0e9
+        assert p0 >= p2 * 0.98 and p2 >= p1 * 0.98
+
+
 def test_two_photon_cross_section_closed_form_on_gpu(hg):
     """Pin P11 through the CUDA path: gen (eta cut only) -> amp2 -> reduce vs the closed form."""
     h = Heget(0, workloads.ALPHA, workloads.Q_U, 0.0, 2.5, 0.0)
