@@ -13,6 +13,7 @@ Functions (all citations are PAPER.md lines, see the C sources):
   philox4x32_10(ctr, key), uniforms(seed, event, slot), phase_space_volume(n, s)
   helicity_bits(seed, event, n), amp2_sampled(seed, momenta, ...)   one random helicity per event
   histogram(momenta, value, observable, lo, hi, nbins)              Fig. 2 distributions
+  helas_wavefunction(fn, p, nhel, ns), helas_vertex(fn, ...)        the HEGET set of Tables 3, 4 as cmplx w[6]
 """
 import ctypes
 import os
@@ -22,7 +23,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libheget_oracle.so")
-_SOURCES = ["heget_oracle.c", "heget_oracle_gen.c", "heget_oracle_next1.c"]
+_SOURCES = ["heget_oracle.c", "heget_oracle_gen.c", "heget_oracle_next1.c", "heget_oracle_helas.c"]
 _DEPS = _SOURCES + ["amp_body.inc"]
 _lib = None
 
@@ -88,6 +89,10 @@ def _load():
     lib.heget_oracle_histogram.argtypes = [dp, dp, ctypes.c_int, ctypes.c_int64, ctypes.c_int, ctypes.c_double,
                                            ctypes.c_double, ctypes.c_int, dp]
     lib.heget_oracle_histogram.restype = None
+    lib.heget_oracle_helas_wavefunction.argtypes = [ctypes.c_int, dp, ctypes.c_int, ctypes.c_int, dp]
+    lib.heget_oracle_helas_wavefunction.restype = None
+    lib.heget_oracle_helas_vertex.argtypes = [ctypes.c_int, dp, dp, dp, ctypes.c_double, dp]
+    lib.heget_oracle_helas_vertex.restype = None
     _lib = lib
     return lib
 
@@ -228,3 +233,33 @@ def histogram(momenta, value, observable, lo, hi, nbins):
     lib.heget_oracle_histogram(_dptr(momenta), _dptr(value), n, N, int(observable), float(lo), float(hi),
                                int(nbins), _dptr(hist))
     return hist
+
+
+# the HEGET function set of Tables 3 and 4; same numbering as include/heget.h
+FN_IXXXX0, FN_IXXXX1, FN_IXXXX2, FN_OXXXX0, FN_OXXXX1, FN_OXXXX2, FN_VXXXX0, FN_VXXXX1, FN_VXXXX2 = range(9)
+VTX_IOVXXX, VTX_FVIXX0, VTX_FVOXX0, VTX_JIOXX0 = range(4)
+
+
+def helas_wavefunction(fn, p, nhel, ns):
+    """cmplx w[6] of ixxxxk / oxxxxk / vxxxxk: components 0..3 and the flowing momentum in 4, 5."""
+    p = np.ascontiguousarray(p, dtype=np.float64)
+    out = np.zeros(12, dtype=np.float64)
+    _load().heget_oracle_helas_wavefunction(int(fn), _dptr(p), int(nhel), int(ns), _dptr(out))
+    return out[0::2] + 1j * out[1::2]
+
+
+def _w12(w):
+    if w is None:
+        return None, None
+    a = np.zeros(12, dtype=np.float64)
+    a[0::2], a[1::2] = np.real(w), np.imag(w)
+    return a, _dptr(a)
+
+
+def helas_vertex(fn, fi=None, fo=None, vc=None, g=G_DEFAULT):
+    """iovxxx(fi,fo,vc) -> complex amplitude; fvixx0(fi,vc), fvoxx0(fo,vc), jioxx0(fi,fo) -> w[6]."""
+    (a, pa), (b, pb), (c, pc) = _w12(fi), _w12(fo), _w12(vc)
+    out = np.zeros(12, dtype=np.float64)
+    _load().heget_oracle_helas_vertex(int(fn), pa, pb, pc, float(g), _dptr(out))
+    w = out[0::2] + 1j * out[1::2]
+    return w[0] if fn == VTX_IOVXXX else w
