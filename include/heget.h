@@ -146,6 +146,32 @@ enum { HEGET_OBS_PT_MAX = 0, HEGET_OBS_DR_MIN = 1, HEGET_OBS_DR_ALL = 2 };
 int heget_histogram(heget_ctx* ctx, const double* momenta, const double* value, int n, int64_t N,
                     int observable, double lo, double hi, int nbins, double* hist, void* stream);
 
+/* The complete HEGET function set of Tables 3 and 4, batched: one call evaluates
+ * one function on N inputs.  A wavefunction is cmplx w[6] = double[6][2]: components 0..3 the
+ * 4-spinor / 4-vector, w[4] = (p0, p3) * nS and w[5] = (p1, p2) * nS the flowing momentum
+ * (PAPER.md:553-554).  Massless, branch-free; "0" = generic direction (spinors: p0 + p3 > 0;
+ * vectors: pT > 0), "1" = momentum along +z, "2" = along -z (only p[0] is read).
+ *   heget_helas_wavefunction: fn = HEGET_FN_*; p [dev] const double[N][4] = (E,px,py,pz);
+ *     nhel = +-1 (twice the helicity / the helicity), ns = nSF or nSV = +-1 (PAPER.md:474-487,
+ *     eqs. 11-13); w [dev] double[N][6][2], written.
+ *   heget_helas_vertex: fn = HEGET_VTX_*; gal[0] = gal[1] = g (eq. 26);
+ *     IOVXXX(fi,fo,vc) -> out [dev] double[N][2], the amplitude g <fo|vc-slash|fi>
+ *     FVIXX0(fi,vc)    -> out [dev] double[N][6][2], -g pf-slash vc-slash |fi> / pf^2, pf = p_fi - p_vc
+ *     FVOXX0(fo,vc)    -> out [dev] double[N][6][2], -g <fo| vc-slash pf-slash / pf^2, pf = p_fo + p_vc
+ *     JIOXX0(fi,fo)    -> out [dev] double[N][6][2], g <fo|gamma^mu|fi> / q^2, q = p_fo - p_fi
+ *     (PAPER.md:622-672); the argument a function does not take may be NULL.
+ * precision selects the arithmetic; all pointers 16-byte aligned; errors as for heget_amp2. */
+enum {
+    HEGET_FN_IXXXX0 = 0, HEGET_FN_IXXXX1 = 1, HEGET_FN_IXXXX2 = 2,
+    HEGET_FN_OXXXX0 = 3, HEGET_FN_OXXXX1 = 4, HEGET_FN_OXXXX2 = 5,
+    HEGET_FN_VXXXX0 = 6, HEGET_FN_VXXXX1 = 7, HEGET_FN_VXXXX2 = 8
+};
+enum { HEGET_VTX_IOVXXX = 0, HEGET_VTX_FVIXX0 = 1, HEGET_VTX_FVOXX0 = 2, HEGET_VTX_JIOXX0 = 3 };
+int heget_helas_wavefunction(heget_ctx* ctx, int fn, int precision, const double* p, int nhel, int ns,
+                             double* w, int64_t N, void* stream);
+int heget_helas_vertex(heget_ctx* ctx, int fn, int precision, const double* fi, const double* fo,
+                       const double* vc, double g, double* out, int64_t N, void* stream);
+
 /* Step 6 of PAPER.md:141 on the device: with x_e = weight[e] * amp2[e] * (1/4)(1/9)(1/n!)
  * (helicity average, colour factor and identical-photon factor of eq. 2, PAPER.md:37;
  * DESIGN.md R1 for the colour factor),

@@ -14,10 +14,12 @@ LIB_PATH = os.path.join(_HERE, "libheget.so")
 FP32, FP64 = 0, 1
 ALGO_TREE, ALGO_SUBSET, ALGO_TREE2 = 0, 1, 2
 OBS_PT_MAX, OBS_DR_MIN, OBS_DR_ALL = 0, 1, 2
+FN_IXXXX0, FN_IXXXX1, FN_IXXXX2, FN_OXXXX0, FN_OXXXX1, FN_OXXXX2, FN_VXXXX0, FN_VXXXX1, FN_VXXXX2 = range(9)
+VTX_IOVXXX, VTX_FVIXX0, VTX_FVOXX0, VTX_JIOXX0 = range(4)
 GEN_FIXED, GEN_LOGUNIFORM, GEN_TOYPDF = 0, 1, 2
 
 EXPORTS = ["heget_init", "heget_destroy", "heget_strerror", "heget_last_cuda_error", "heget_rambo",
-           "heget_gen_events", "heget_amp2", "heget_amp2_algo", "heget_amp2_sampled", "heget_histogram", "heget_xsec_reduce", "heget_xsec_host", "heget_fma_peak", "heget_fma_peak_pattern",
+           "heget_gen_events", "heget_amp2", "heget_amp2_algo", "heget_amp2_sampled", "heget_histogram", "heget_helas_wavefunction", "heget_helas_vertex", "heget_xsec_reduce", "heget_xsec_host", "heget_fma_peak", "heget_fma_peak_pattern",
            "heget_launch_count"]
 
 
@@ -64,6 +66,10 @@ def load_library():
     lib.heget_amp2_sampled.restype = ci
     lib.heget_histogram.argtypes = [vp, dp, dp, ci, i64, ci, cd, cd, ci, dp, vp]
     lib.heget_histogram.restype = ci
+    lib.heget_helas_wavefunction.argtypes = [vp, ci, ci, dp, ci, ci, dp, i64, vp]
+    lib.heget_helas_wavefunction.restype = ci
+    lib.heget_helas_vertex.argtypes = [vp, ci, ci, dp, dp, dp, cd, dp, i64, vp]
+    lib.heget_helas_vertex.restype = ci
     lib.heget_xsec_reduce.argtypes = [vp, dp, dp, ci, i64, dp, vp]
     lib.heget_xsec_reduce.restype = ci
     lib.heget_xsec_host.argtypes = [vp, dp, dp, ci, ci, i64, dp, dp]
@@ -177,6 +183,29 @@ class Heget:
                                               lo, hi, nbins, hist.data_ptr(), _stream_ptr(self.device)),
                     "heget_histogram")
         return hist
+
+    def helas_wavefunction(self, fn, p, nhel, ns, precision=FP64):
+        """ixxxxk / oxxxxk / vxxxxk on p[N][4] -> w[N][6][2] (cmplx w[6])."""
+        _check_dev(p, None, self.device)
+        if p.dim() != 2 or p.shape[1] != 4:
+            raise HegetError("p must be [N][4]")
+        w = torch.empty((p.shape[0], 6, 2), dtype=torch.float64, device=self.device)
+        self._check(self._lib.heget_helas_wavefunction(self._ctx, fn, precision, p.data_ptr(), nhel, ns,
+                                                       w.data_ptr(), p.shape[0], _stream_ptr(self.device)),
+                    "heget_helas_wavefunction")
+        return w
+
+    def helas_vertex(self, fn, fi=None, fo=None, vc=None, g=0.0, precision=FP64):
+        """iovxxx -> [N][2]; fvixx0 / fvoxx0 / jioxx0 -> [N][6][2]."""
+        given = [t for t in (fi, fo, vc) if t is not None]
+        for t in given:
+            _check_dev(t, (given[0].shape[0], 6, 2), self.device)
+        N = given[0].shape[0]
+        out = torch.empty((N, 2) if fn == VTX_IOVXXX else (N, 6, 2), dtype=torch.float64, device=self.device)
+        ptr = lambda t: t.data_ptr() if t is not None else None  # noqa: E731
+        self._check(self._lib.heget_helas_vertex(self._ctx, fn, precision, ptr(fi), ptr(fo), ptr(vc), g,
+                                                 out.data_ptr(), N, _stream_ptr(self.device)), "heget_helas_vertex")
+        return out
 
     def xsec_reduce(self, amp2, weight, n, out3=None):
         _check_dev(amp2, None, self.device)

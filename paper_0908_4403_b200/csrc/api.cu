@@ -196,6 +196,41 @@ int heget_histogram(heget_ctx* ctx, const double* momenta, const double* value, 
     return err == cudaSuccess ? HEGET_OK : fail_cuda(ctx, err);
 }
 
+int heget_helas_wavefunction(heget_ctx* ctx, int fn, int precision, const double* p, int nhel, int ns, double* w,
+                               int64_t N, void* stream)
+{
+    if (!ctx || N < 0 || (N > 0 && (!p || !w))) return HEGET_EINVAL;
+    if (fn < HEGET_FN_IXXXX0 || fn > HEGET_FN_VXXXX2) return HEGET_EINVAL;
+    if (precision != HEGET_FP32 && precision != HEGET_FP64) return HEGET_EINVAL;
+    if ((nhel != 1 && nhel != -1) || (ns != 1 && ns != -1)) return HEGET_EINVAL;
+    if (((reinterpret_cast<uintptr_t>(p) | reinterpret_cast<uintptr_t>(w)) & 15u) != 0) return HEGET_EINVAL;
+    DeviceGuard guard(ctx->device);
+    if (!guard.ok) return fail_cuda(ctx, cudaGetLastError());
+    int launches = 0;
+    cudaError_t err = heget_launch_helas_wavefunction(fn, precision, p, nhel, ns, w, N, (cudaStream_t)stream, &launches);
+    ctx->launches += launches;
+    return err == cudaSuccess ? HEGET_OK : fail_cuda(ctx, err);
+}
+
+int heget_helas_vertex(heget_ctx* ctx, int fn, int precision, const double* fi, const double* fo, const double* vc,
+                       double g, double* out, int64_t N, void* stream)
+{
+    if (!ctx || N < 0 || (N > 0 && !out)) return HEGET_EINVAL;
+    if (fn < HEGET_VTX_IOVXXX || fn > HEGET_VTX_JIOXX0) return HEGET_EINVAL;
+    if (precision != HEGET_FP32 && precision != HEGET_FP64) return HEGET_EINVAL;
+    const bool need_fi = fn != HEGET_VTX_FVOXX0, need_fo = fn != HEGET_VTX_FVIXX0, need_vc = fn != HEGET_VTX_JIOXX0;
+    if (N > 0 && ((need_fi && !fi) || (need_fo && !fo) || (need_vc && !vc))) return HEGET_EINVAL;
+    if (((reinterpret_cast<uintptr_t>(fi) | reinterpret_cast<uintptr_t>(fo) | reinterpret_cast<uintptr_t>(vc) |
+          reinterpret_cast<uintptr_t>(out)) & 15u) != 0)
+        return HEGET_EINVAL;
+    DeviceGuard guard(ctx->device);
+    if (!guard.ok) return fail_cuda(ctx, cudaGetLastError());
+    int launches = 0;
+    cudaError_t err = heget_launch_helas_vertex(fn, precision, fi, fo, vc, g, out, N, (cudaStream_t)stream, &launches);
+    ctx->launches += launches;
+    return err == cudaSuccess ? HEGET_OK : fail_cuda(ctx, err);
+}
+
 int heget_xsec_reduce(heget_ctx* ctx, const double* amp2, const double* weight, int n, int64_t N, double* out3,
                       void* stream)
 {

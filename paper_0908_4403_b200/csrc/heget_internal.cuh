@@ -44,6 +44,10 @@ cudaError_t heget_launch_amp2_sampled(const heget_ctx* ctx, uint64_t seed, uint6
 cudaError_t heget_launch_histogram(const heget_ctx* ctx, const double* momenta, const double* value, int n,
                                    int64_t N, int observable, double lo, double hi, int nbins, double* hist,
                                    cudaStream_t stream, int* launches);
+cudaError_t heget_launch_helas_wavefunction(int fn, int precision, const double* p, int nhel, int ns, double* out,
+                                            int64_t N, cudaStream_t stream, int* launches);
+cudaError_t heget_launch_helas_vertex(int fn, int precision, const double* a, const double* b, const double* c,
+                                      double g, double* out, int64_t N, cudaStream_t stream, int* launches);
 cudaError_t heget_launch_gen(const heget_ctx* ctx, uint64_t seed, int n, const heget_gen_cfg* cfg,
                              uint64_t first_event, int64_t N, double* momenta, double* weight,
                              cudaStream_t stream, int* launches);
