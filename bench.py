@@ -45,6 +45,31 @@ def executed_flops_per_event(n):
     return 2 ** n * (36 * internal + 10 * math.factorial(n))
 
 
+def _binom(n, k):
+    return math.factorial(n) // (math.factorial(k) * math.factorial(n - k))
+
+
+def executed_flops_per_event_algo(n, algo):
+    """Executed flops of the separately named algorithms, tables excluded.
+    subset: level m holds C(n,m) 2^m items of m vertex accumulations (8 FMA + 4 ADD = 20 flop) and
+    one propagator (8 FMA + 4 MUL = 20 flop); 2^n closings of n terms (4 FMA + 2 ADD = 10 flop).
+    two-sided: per lane the tree to depth n-KS (36 flop per node) and n!/KS! closings (16 flop),
+    plus the ubar-side table, C(n,m) 2^m entries of m x 40 flop for m = 2..KS, KS = min(n,3)."""
+    if algo == "tree":
+        return executed_flops_per_event(n)
+    if algo == "subset":
+        return sum(_binom(n, m) * 2 ** m * (20 * m + 20) for m in range(1, n)) + 2 ** n * 10 * n
+    ks = min(n, 3)
+    nodes = sum(math.factorial(n) // math.factorial(n - l) for l in range(1, n - ks + 1))
+    per_lane = 36 * nodes + 16 * (math.factorial(n) // math.factorial(ks))
+    table = sum(_binom(n, m) * 2 ** m * m * 40 for m in range(2, ks + 1))
+    return 2 ** n * per_lane + table
+
+
+ALGOS = {"tree": 0, "subset": 1, "two-sided": 2}
+KERNEL_NAME = {"tree": "amp2_kernel", "subset": "amp2_subset_kernel", "two-sided": "amp2_twosided_kernel"}
+
+
 def theoretical_peak(precision, sm_count, sm_max_mhz):
     lanes = 128 if precision == "fp32" else 64       # FP32 / FP64 FMA lanes per SM on B200
     return sm_count * lanes * 2 * sm_max_mhz * 1e6
@@ -168,6 +193,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="4gamma")
     ap.add_argument("--precision", default="fp64", choices=["fp32", "fp64"])
+    ap.add_argument("--algo", default="tree", choices=sorted(ALGOS),
+                    help="organisation of the permutation sum timed in the headline line (heget_amp2_algo); "
+                         "tree = the north-star method and the default")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-sweep", action="store_true", help="skip the per-n / per-precision table")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -221,7 +249,8 @@ def main():
     launches0 = hg.launch_count()
     sampler = ClockSampler(local_rank)
     sampler.start()
-    total_ms, amp_ms, amp_ms_best, sums, nl = timed_run(args.config, args.precision, args.steps, args.warmup)
+    total_ms, amp_ms, amp_ms_best, sums, nl = timed_run(args.config, args.precision, args.steps, args.warmup,
+                                                         algo=ALGOS[args.algo])
     clocks = sampler.stop()
     launches = hg.launch_count() - launches0 - 3 * args.warmup - 1   # minus warm-up steps and the generator
     if world > 1:
@@ -268,13 +297,13 @@ def main():
     peak_node = hg.fma_peak(prec, 2)
     sm_max = clocks["sm_max_mhz"] or 1965.0
     peak_theory = theoretical_peak(args.precision, torch.cuda.get_device_properties(local_rank).multi_processor_count, sm_max)
-    achieved = executed_flops_per_event(n) * nl / (amp_ms * 1e-3)
+    achieved = executed_flops_per_event_algo(n, args.algo) * nl / (amp_ms * 1e-3)
     model_c = model_flops_per_event(n) * nl / (amp_ms * 1e-3)
     roofline = {"bound": "alu", "achieved": achieved / 1e12, "peak": peak_measured / 1e12, "unit": "TFLOP/s",
-                "frac": achieved / peak_measured, "traffic": NCU_DRAM_BYTES.get((n, args.precision)),
-                "kernel": "amp2_kernel<%d,%s>" % (n, "double" if prec == FP64 else "float"),
+                "frac": achieved / peak_measured, "traffic": NCU_DRAM_BYTES.get((n, args.precision)) if args.algo == "tree" else None,
+                "kernel": "%s<%d,%s>" % (KERNEL_NAME[args.algo], n, "double" if prec == FP64 else "float"),
                 "kernel_ms": amp_ms, "kernel_ms_best": amp_ms_best,
-                "flops_per_event_executed": executed_flops_per_event(n),
+                "flops_per_event_executed": executed_flops_per_event_algo(n, args.algo),
                 "peak_source": "heget_fma_peak on this GPU: FMA with constant-bank operands "
                                "(MEASURED_PEAKS.json has no non-tensor figure)",
                 "peak_theoretical": peak_theory / 1e12, "frac_of_theoretical": achieved / peak_theory,
@@ -289,7 +318,7 @@ def main():
               "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
               "scaling": "weak", "vs_baseline": None, "dtype": "f64" if prec == FP64 else "f32",
               "data": "synthetic",
-              "config": {"workload": args.config, "n_photons": n, "events_per_gpu": nl,
+              "config": {"workload": args.config, "n_photons": n, "events_per_gpu": nl, "algo": args.algo,
                          "generation": "device Philox4x32-10 + RAMBO, seed %d" % cfg["seed"],
                          "l2": "256 MiB buffer written between timed steps (L2 flush)"},
               "clocks": clocks,
@@ -318,13 +347,31 @@ def main():
                         (2, "two-sided", "HEGET_ALGO_TREE2 (heget_amp2_algo): tree from u to depth n-3, closed with "
                                          "row vectors chained from ubar; own flop count")):
                     _, s_ms, _, _, _ = timed_run(name, precision, 3, 3, algo=algo_id)
+                    s_fl = executed_flops_per_event_algo(nph, algo_name) * nn / (s_ms * 1e-3)
                     table.append({"workload": name, "n": nph, "precision": precision, "events": nn, "algo": algo_name,
-                                  "amp2_ms": s_ms, "events_per_s": nn / (s_ms * 1e-3), "note": note})
+                                  "amp2_ms": s_ms, "events_per_s": nn / (s_ms * 1e-3),
+                                  "executed_tflops": s_fl / 1e12, "frac_of_measured_peak": s_fl / pk, "note": note})
                 table.append({"workload": name, "n": nph, "precision": precision, "events": nn, "algo": "tree",
                               "amp2_ms": a_ms, "events_per_s": nn / (a_ms * 1e-3),
                               "executed_tflops": ach / 1e12, "frac_of_measured_peak": ach / pk,
                               "model_c_tflops": model_flops_per_event(nph) * nn / (a_ms * 1e-3) / 1e12})
         result["per_config"] = table
+
+    if not args.no_sweep and world == 1:
+        # NEXT-1 entry points on the headline workload: one drawn helicity per event, Fig. 2 histogram
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        val, _ = hg.amp2_sampled(cfg["seed"], mom_d, prec)
+        hg.histogram(mom_d, val, 0, 0.0, 1500.0, 60)
+        torch.cuda.synchronize()
+        ev[0].record()
+        val, _ = hg.amp2_sampled(cfg["seed"], mom_d, prec)
+        ev[1].record()
+        hg.histogram(mom_d, val, 0, 0.0, 1500.0, 60)
+        ev[2].record()
+        torch.cuda.synchronize()
+        result["next1"] = {"amp2_sampled_ms": ev[0].elapsed_time(ev[1]),
+                           "amp2_sampled_events_per_s": nl / (ev[0].elapsed_time(ev[1]) * 1e-3),
+                           "histogram_ms": ev[1].elapsed_time(ev[2]), "events": nl, "precision": args.precision}
 
     print(json.dumps(result))
     hg.close()
