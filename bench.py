@@ -54,12 +54,12 @@ def executed_flops_per_event_algo(n, algo):
     subset: level m holds C(n,m) 2^m items of m vertex accumulations (8 FMA + 4 ADD = 20 flop) and
     one propagator (8 FMA + 4 MUL = 20 flop); 2^n closings of n terms (4 FMA + 2 ADD = 10 flop).
     two-sided: per lane the tree to depth n-KS (36 flop per node) and n!/KS! closings (16 flop),
-    plus the ubar-side table, C(n,m) 2^m entries of m x 40 flop for m = 2..KS, KS = min(n,3)."""
+    plus the ubar-side table, C(n,m) 2^m entries of m x 40 flop for m = 2..KS, KS = min(n,4)."""
     if algo == "tree":
         return executed_flops_per_event(n)
     if algo == "subset":
         return sum(_binom(n, m) * 2 ** m * (20 * m + 20) for m in range(1, n)) + 2 ** n * 10 * n
-    ks = min(n, 3)
+    ks = min(n, 4)
     nodes = sum(math.factorial(n) // math.factorial(n - l) for l in range(1, n - ks + 1))
     per_lane = 36 * nodes + 16 * (math.factorial(n) // math.factorial(ks))
     table = sum(_binom(n, m) * 2 ** m * m * 40 for m in range(2, ks + 1))
@@ -344,7 +344,7 @@ def main():
                 ach = executed_flops_per_event(nph) * nn / (a_ms * 1e-3)
                 for algo_id, algo_name, note in (
                         (1, "subset", "HEGET_ALGO_SUBSET (heget_amp2_algo): not the permutation tree, own flop count"),
-                        (2, "two-sided", "HEGET_ALGO_TREE2 (heget_amp2_algo): tree from u to depth n-3, closed with "
+                        (2, "two-sided", "HEGET_ALGO_TREE2 (heget_amp2_algo): tree from u to depth n-4, closed with "
                                          "row vectors chained from ubar; own flop count")):
                     _, s_ms, _, _, _ = timed_run(name, precision, 3, 3, algo=algo_id)
                     s_fl = executed_flops_per_event_algo(nph, algo_name) * nn / (s_ms * 1e-3)

@@ -7,22 +7,25 @@
 //   * from the ubar end, the row vectors
 //         L_1[j]   = <vbar| E'_j                                        (closing vertex, no propagator)
 //         L_m+1[T] = sum_{x in T} ( L_m[T \ x] P_{all \ (T \ x)} ) E'_x    (fvoxx0 summed over orderings)
-//     are tabulated in shared memory for all sets T of up to KS = min(n, 3) photons and all
-//     helicities of T (C(n,2) 4 + C(n,3) 8 entries; n = 8: 560);
+//     are tabulated in shared memory for all sets T of up to KS = min(n, 4) photons and all
+//     helicities of T (C(n,2) 4 + C(n,3) 8 + C(n,4) 16 entries; n = 8: 1 680);
 //   * from the u end, the depth-first permutation tree of amp2.cu is walked only to depth n - KS
 //     (each ordered prefix once), and every node at that depth closes with ONE dot product
 //         ampsum += L_KS[remaining photons] . psi
 //     instead of the KS! orderings below it.
 // Per helicity configuration: sum_{l=1}^{n-KS} n!/(n-l)! fvixx0 nodes and n!/KS! closings
-// (n = 8: 8 800 + 6 720 against 69 280 + 40 320 in the one-sided tree).  Same E' / P tables,
+// (n = 8: 2 080 + 1 680 against 69 280 + 40 320 in the one-sided tree).  Same E' / P tables,
 // parity shortcut, lane mapping (one lane per helicity configuration) and epilogue as amp2.cu.
 #include "amp2_tree.cuh"
 #include "subset_index.cuh"
 
 namespace {
 
+#ifndef HEGET_KSUFFIX
+#define HEGET_KSUFFIX 4
+#endif
 template <int N>
-constexpr int kSuffix = (N < 3) ? N : 3;  // KS: photons attached from the ubar end
+constexpr int kSuffix = (N < HEGET_KSUFFIX) ? N : HEGET_KSUFFIX;  // KS: photons attached from the ubar end
 
 // row vector times the propagator block, r' = r P,  P = [[pp, px - i py], [px + i py, pm]]
 template <typename T>
@@ -166,9 +169,11 @@ struct TwoSidedSmem {
     static constexpr int MOM = 4 * (N + 2);
     static constexpr int L2 = binom(N, 2) << 2;                 // entries of level 2
     static constexpr int L3 = (KS >= 3) ? (binom(N, 3) << 3) : 0;  // entries of level 3
+    static constexpr int L4 = (KS >= 4) ? (binom(N, 4) << 4) : 0;  // entries of level 4
     static constexpr size_t off_l2 = 0;
     static constexpr size_t off_l3 = off_l2 + sizeof(Spinor<T>) * G::EPB * L2;
-    static constexpr size_t off_P = off_l3 + sizeof(Spinor<T>) * G::EPB * L3;
+    static constexpr size_t off_l4 = off_l3 + sizeof(Spinor<T>) * G::EPB * L3;
+    static constexpr size_t off_P = off_l4 + sizeof(Spinor<T>) * G::EPB * L4;
     static constexpr size_t off_E = off_P + sizeof(PEntry<T>) * G::EPB * G::L;
     static constexpr size_t off_mom = off_E + sizeof(EEntry<T>) * G::EPB * 2 * N;
     static constexpr size_t off_s2 = off_mom + sizeof(double) * G::EPB * MOM;
@@ -178,8 +183,11 @@ struct TwoSidedSmem {
     static constexpr size_t bytes = off_list + (N + 1) * 72;
 };
 
+#ifndef HEGET_TS_MINB64
+#define HEGET_TS_MINB64 1
+#endif
 template <int N, typename T>
-__global__ void __launch_bounds__(Geometry<N>::THREADS, (sizeof(T) == 4) ? 1 : 2)
+__global__ void __launch_bounds__(Geometry<N>::THREADS, (sizeof(T) == 4) ? 1 : HEGET_TS_MINB64)
 amp2_twosided_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_t n_events, double g)
 {
     using G = Geometry<N>;
@@ -189,6 +197,7 @@ amp2_twosided_kernel(const double* __restrict__ momenta, double* __restrict__ ou
     extern __shared__ __align__(32) unsigned char smem[];
     Spinor<T>* s_l2 = reinterpret_cast<Spinor<T>*>(smem + SM::off_l2);
     Spinor<T>* s_l3 = reinterpret_cast<Spinor<T>*>(smem + SM::off_l3);
+    Spinor<T>* s_l4 = reinterpret_cast<Spinor<T>*>(smem + SM::off_l4);
     PEntry<T>* s_P = reinterpret_cast<PEntry<T>*>(smem + SM::off_P);
     EEntry<T>* s_E = reinterpret_cast<EEntry<T>*>(smem + SM::off_E);
     double* s_mom = reinterpret_cast<double*>(smem + SM::off_mom);
@@ -208,13 +217,18 @@ amp2_twosided_kernel(const double* __restrict__ momenta, double* __restrict__ ou
     const EEntry<T>* E = s_E + ev_local * 2 * N;
     Spinor<T>* l2 = s_l2 + ev_local * SM::L2;
     Spinor<T>* l3 = s_l3 + ev_local * SM::L3;
+    Spinor<T>* l4 = s_l4 + ev_local * SM::L4;
     build_suffix_level<N, 2, T>(P, E, s_rank, s_list, nullptr, l2, hel);
     __syncthreads();
     if constexpr (KS >= 3) {
         build_suffix_level<N, 3, T>(P, E, s_rank, s_list, l2, l3, hel);
         __syncthreads();
     }
-    const Spinor<T>* Ltab = (KS >= 3) ? l3 : l2;
+    if constexpr (KS >= 4) {
+        build_suffix_level<N, 4, T>(P, E, s_rank, s_list, l3, l4, hel);
+        __syncthreads();
+    }
+    const Spinor<T>* Ltab = (KS >= 4) ? l4 : (KS >= 3) ? l3 : l2;
 
     T ar = 0, ai = 0;
     const Spinor<T> f0 = {(T)1, (T)0, (T)0, (T)0};
