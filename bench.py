@@ -112,12 +112,17 @@ class ClockSampler:
                 "reasons": reasons, "samples": len(self.rows)}
 
 
-def oracle_sample_events(cfg, seconds_budget=15.0):
-    """How many events of this config the oracle is timed on (bounded CPU work)."""
-    per_event_core_s = {2: 2e-6, 3: 2.5e-5, 4: 2.4e-4, 5: 3.3e-3, 6: 5e-2, 7: 0.8, 8: 13.0}[cfg["n"]] * 8
+def oracle_sample_events(cfg, seconds_budget=12.0):
+    """How many events of this config the oracle is timed on: a BOUNDED sample sized for about
+    `seconds_budget` seconds of wall time on this host (10-30 s of CPU work on all its cores),
+    from a one-second pilot run of the oracle itself."""
     cores = os.cpu_count() or 1
-    want = int(seconds_budget * cores / per_event_core_s)
-    return max(min(want, cfg["oracle_events"], cfg["N"]), min(cores, 4))
+    per_event_core_s = {2: 2e-6, 3: 2.5e-5, 4: 1e-4, 5: 1.5e-3, 6: 2.5e-2, 7: 0.4, 8: 6.0}[cfg["n"]]
+    pilot = max(min(int(1.0 * cores / per_event_core_s), cfg["N"]), 1)
+    rate, _, _ = time_oracle(cfg, pilot)
+    want = int(rate * seconds_budget)
+    # at least one event (the oracle spreads a single event's helicity assignments over the cores)
+    return max(min(want, cfg["N"]), 1)
 
 
 def time_oracle(cfg, n_events):
