@@ -36,27 +36,39 @@ def model_flops_per_event(n):
     return 2 * 2 ** n * (44 * internal + 24 * math.factorial(n))
 
 
-def executed_flops_per_event(n):
-    """What amp2_kernel executes (DESIGN.md section 6): 2^n lanes (sigma_1 = +1 only, doubled by
+def executed_flops_per_event(n, precision="fp32"):
+    """What amp2_kernel executes (DESIGN.md section 6.1): 2^n lanes (sigma_1 = +1 only, doubled by
     parity), per lane one fvixx0 node = 16 FMA + 4 MUL = 36 flop per ordered prefix and one iovxxx
-    leaf = 4 FMA + 2 ADD = 10 flop per permutation.  Cross-checked against ncu's
+    leaf = 4 FMA + 2 ADD = 10 flop per permutation.  The fp64 kernels share spinors between
+    helicity lanes: for n <= 7 the two lanes that differ in the last photon's helicity compute one
+    of the two last-level nodes each and exchange them by shuffle whenever both remaining photons
+    have index < 5 (a fraction C(min(n,5),2)/C(n,2) of the n!/2 last-but-one nodes saves one node);
+    the 4-photon kernel also computes the first two tree levels once per event (48 two-node
+    entries) instead of once per lane (16 nodes).  Tables excluded.  Cross-checked against ncu's
     sass_thread_inst_executed_op_{f,d}{fma,mul,add} counters in profiles/."""
     internal = sum(math.factorial(n) // math.factorial(n - l) for l in range(1, n))
-    return 2 ** n * (36 * internal + 10 * math.factorial(n))
+    flops = 2 ** n * (36 * internal + 10 * math.factorial(n))
+    if precision == "fp64" and 2 <= n <= 7:
+        m = min(n, 5)
+        share = (m * (m - 1) // 2) / (n * (n - 1) // 2)
+        flops -= 2 ** n * (math.factorial(n) // 2) * share * 36
+        if n == 4:
+            flops -= 2 ** n * 16 * 36 - 48 * 2 * 36
+    return flops
 
 
 def _binom(n, k):
     return math.factorial(n) // (math.factorial(k) * math.factorial(n - k))
 
 
-def executed_flops_per_event_algo(n, algo):
+def executed_flops_per_event_algo(n, algo, precision="fp32"):
     """Executed flops of the separately named algorithms, tables excluded.
     subset: level m holds C(n,m) 2^m items of m vertex accumulations (8 FMA + 4 ADD = 20 flop) and
     one propagator (8 FMA + 4 MUL = 20 flop); 2^n closings of n terms (4 FMA + 2 ADD = 10 flop).
     two-sided: per lane the tree to depth n-KS (36 flop per node) and n!/KS! closings (16 flop),
     plus the ubar-side table, C(n,m) 2^m entries of m x 40 flop for m = 2..KS, KS = min(n,4)."""
     if algo == "tree":
-        return executed_flops_per_event(n)
+        return executed_flops_per_event(n, precision)
     if algo == "subset":
         return sum(_binom(n, m) * 2 ** m * (20 * m + 20) for m in range(1, n)) + 2 ** n * 10 * n
     ks = min(n, 4)
@@ -302,21 +314,22 @@ def main():
     peak_node = hg.fma_peak(prec, 2)
     sm_max = clocks["sm_max_mhz"] or 1965.0
     peak_theory = theoretical_peak(args.precision, torch.cuda.get_device_properties(local_rank).multi_processor_count, sm_max)
-    achieved = executed_flops_per_event_algo(n, args.algo) * nl / (amp_ms * 1e-3)
+    achieved = executed_flops_per_event_algo(n, args.algo, args.precision) * nl / (amp_ms * 1e-3)
     model_c = model_flops_per_event(n) * nl / (amp_ms * 1e-3)
     roofline = {"bound": "alu", "achieved": achieved / 1e12, "peak": peak_measured / 1e12, "unit": "TFLOP/s",
                 "frac": achieved / peak_measured, "traffic": NCU_DRAM_BYTES.get((n, args.precision)) if args.algo == "tree" else None,
                 "kernel": "%s<%d,%s>" % (KERNEL_NAME[args.algo], n, "double" if prec == FP64 else "float"),
                 "kernel_ms": amp_ms, "kernel_ms_best": amp_ms_best,
-                "flops_per_event_executed": executed_flops_per_event_algo(n, args.algo),
+                "flops_per_event_executed": executed_flops_per_event_algo(n, args.algo, args.precision),
                 "peak_source": "heget_fma_peak on this GPU: FMA with constant-bank operands "
                                "(MEASURED_PEAKS.json has no non-tensor figure)",
                 "peak_theoretical": peak_theory / 1e12, "frac_of_theoretical": achieved / peak_theory,
                 "peak_three_register_fma": peak_3reg / 1e12, "peak_node_pattern": peak_node / 1e12,
                 "frac_of_node_pattern": achieved / peak_node,
                 "model_c_tflops": model_c / 1e12, "model_c_frac": model_c / peak_measured,
-                "flops_model": "executed: 2^n lanes x (36 flop per tree node + 10 per leaf); model C (SURVEY 8(d)): "
-                               "2*2^n x (44 per node + 24 per leaf), about 2.5x the executed count because the kernel "
+                "flops_model": "executed: 2^n lanes x (36 flop per tree node + 10 per leaf), minus the nodes the fp64 "
+                               "kernels share between helicity lanes (see executed_flops_per_event); model C (SURVEY "
+                               "8(d)): 2*2^n x (44 per node + 24 per leaf), 2.5-5x the executed count because the kernel "
                                "evaluates sigma_1=+1 only (parity) with normalised polarisation blocks"}
 
     result = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -346,13 +359,13 @@ def main():
                 _, a_ms, a_best, _, nn = timed_run(name, precision, 3, 3)
                 nph = workloads.CONFIGS[name]["n"]
                 pk = peak_measured if precision == args.precision else hg.fma_peak(FP64 if precision == "fp64" else FP32)
-                ach = executed_flops_per_event(nph) * nn / (a_ms * 1e-3)
+                ach = executed_flops_per_event(nph, precision) * nn / (a_ms * 1e-3)
                 for algo_id, algo_name, note in (
                         (1, "subset", "HEGET_ALGO_SUBSET (heget_amp2_algo): not the permutation tree, own flop count"),
                         (2, "two-sided", "HEGET_ALGO_TREE2 (heget_amp2_algo): tree from u to depth n-4, closed with "
                                          "row vectors chained from ubar; own flop count")):
                     _, s_ms, _, _, _ = timed_run(name, precision, 3, 3, algo=algo_id)
-                    s_fl = executed_flops_per_event_algo(nph, algo_name) * nn / (s_ms * 1e-3)
+                    s_fl = executed_flops_per_event_algo(nph, algo_name, precision) * nn / (s_ms * 1e-3)
                     table.append({"workload": name, "n": nph, "precision": precision, "events": nn, "algo": algo_name,
                                   "amp2_ms": s_ms, "events_per_s": nn / (s_ms * 1e-3),
                                   "executed_tflops": s_fl / 1e12, "frac_of_measured_peak": s_fl / pk, "note": note})

@@ -3,10 +3,15 @@
 // amp2.cu (all helicities, one lane per helicity configuration) and amp2_sampled.cu (one drawn
 // helicity configuration per event, lanes split the top of the tree).
 #pragma once
+#include <type_traits>
+
 #include "amp2_common.cuh"
 
 #ifndef HEGET_KB
 #define HEGET_KB 4          // unrolled bottom levels of the permutation tree
+#endif
+#ifndef HEGET_SHARE_BY_PTR
+#define HEGET_SHARE_BY_PTR 1  // lane-sharing kernels keep E' entries as pointers (one select instead of eight)
 #endif
 #ifndef HEGET_E_BY_PTR
 #define HEGET_E_BY_PTR 0    // 1: Bottom<K> re-reads E' entries from shared memory instead of holding them
@@ -45,32 +50,74 @@ __device__ __forceinline__ void iovxxx_weyl(const EEntry<T>& E, const Spinor<T>&
 // of a subtree is straight-line FMAs plus one P-entry load per node.
 template <typename T> __device__ __forceinline__ const EEntry<T>& eload(const EEntry<T>& e) { return e; }
 template <typename T> __device__ __forceinline__ EEntry<T> eload(const EEntry<T>* e) { return *e; }
+template <typename T>
+__device__ __forceinline__ EEntry<T> eselect(bool c, const EEntry<T>& a, const EEntry<T>& b)
+{
+    EEntry<T> r;
+    r.ar = c ? a.ar : b.ar; r.ai = c ? a.ai : b.ai; r.br = c ? a.br : b.br; r.bi = c ? a.bi : b.bi;
+    return r;
+}
+template <typename T>
+__device__ __forceinline__ EEntry<T> eselect(bool c, const EEntry<T>* a, const EEntry<T>* b) { return *(c ? a : b); }
 
-template <int K, typename T, typename EA>
+// SHARE = 1 (amp2.cu, fp64): at the last level the two lanes that differ only in the helicity of
+// the photon still to be closed need the SAME off-shell spinor (a prefix's spinor depends on the
+// helicities of the photons in the prefix only).  With two photons a, b left, a lane whose
+// helicity bits of a and b are equal computes psi(.., a) and receives psi(.., b) from the lane
+// with bit a flipped; a lane whose bits differ computes psi(.., b) and receives psi(.., a) from the
+// lane with bit b flipped -- one fvixx0 (20 FP64 instructions) and 8 shuffles per lane instead of
+// two fvixx0.  Every lane still executes the same instruction stream (per-lane operand selects).
+// Needs both photons' lane bits inside the warp (photon index < 5); otherwise, and always for
+// SHARE = 0 (fp32, where the shuffles would cost what they save; amp2_sampled.cu, whose lanes are
+// not helicity configurations), both nodes are computed.  hb[] = this lane's helicity bits.
+template <int K, typename T, typename EA, int SHARE = 0>
 struct Bottom {
     static __device__ __forceinline__ void run(const PEntry<T>* __restrict__ PS, const int (&bit)[K],
-                                               const EA (&e)[K], const Spinor<T>& f, T& ar, T& ai)
+                                               const EA (&e)[K], const unsigned (&hb)[K], const Spinor<T>& f,
+                                               T& ar, T& ai)
     {
+        if constexpr (K == 2 && SHARE == 1) {
+            if ((bit[0] | bit[1]) < 32) {  // uniform over the CTA
+                const bool odd = (hb[0] ^ hb[1]) != 0u;
+                // mine: the photon this lane attaches; other: the one it closes with.  With
+                // pointer lists the choice is one select and a shared-memory load per entry.
+                const EEntry<T> em = eselect<T>(odd, e[1], e[0]);
+                const EEntry<T> eo = eselect<T>(odd, e[0], e[1]);
+                const int bm = odd ? bit[1] : bit[0];
+                const Spinor<T> fm = fvixx0_weyl(PS[bm], em, f);
+                Spinor<T> fo;
+                fo.r0 = __shfl_xor_sync(0xffffffffu, fm.r0, bm);
+                fo.i0 = __shfl_xor_sync(0xffffffffu, fm.i0, bm);
+                fo.r1 = __shfl_xor_sync(0xffffffffu, fm.r1, bm);
+                fo.i1 = __shfl_xor_sync(0xffffffffu, fm.i1, bm);
+                iovxxx_weyl(eo, fm, ar, ai);  // my node closes with the other photon
+                iovxxx_weyl(em, fo, ar, ai);  // the received node closes with my photon
+                return;
+            }
+        }
 #pragma unroll
         for (int i = 0; i < K; ++i) {
             int sub_bit[K - 1];
             EA sub_e[K - 1];
+            unsigned sub_hb[K - 1];
 #pragma unroll
             for (int m = 0; m < K - 1; ++m) {
                 sub_bit[m] = bit[m + (m >= i ? 1 : 0)];
                 sub_e[m] = e[m + (m >= i ? 1 : 0)];
+                sub_hb[m] = hb[m + (m >= i ? 1 : 0)];
             }
             const PEntry<T>* Pn = PS + bit[i];
             const Spinor<T> fn = fvixx0_weyl(*Pn, eload<T>(e[i]), f);
-            Bottom<K - 1, T, EA>::run(Pn, sub_bit, sub_e, fn, ar, ai);
+            Bottom<K - 1, T, EA, SHARE>::run(Pn, sub_bit, sub_e, sub_hb, fn, ar, ai);
         }
     }
 };
 
-template <typename T, typename EA>
-struct Bottom<1, T, EA> {
+template <typename T, typename EA, int SHARE>
+struct Bottom<1, T, EA, SHARE> {
     static __device__ __forceinline__ void run(const PEntry<T>* __restrict__, const int (&)[1],
-                                               const EA (&e)[1], const Spinor<T>& f, T& ar, T& ai)
+                                               const EA (&e)[1], const unsigned (&)[1], const Spinor<T>& f,
+                                               T& ar, T& ai)
     {
         iovxxx_weyl(eload<T>(e[0]), f, ar, ai);
     }
@@ -78,7 +125,7 @@ struct Bottom<1, T, EA> {
 
 // Depth-first walk of the upper levels.  `used` = set of photons already attached (uniform
 // over the CTA); when KB photons remain the unrolled Bottom<KB> takes over.
-template <int N, int DEPTH, int KB, typename T>
+template <int N, int DEPTH, int KB, typename T, int SHARE = 0>
 struct Walk {
     static __device__ __forceinline__ void run(const PEntry<T>* __restrict__ P, const EEntry<T>* __restrict__ E,
                                                unsigned hel, unsigned used, const Spinor<T>& f, T& ar, T& ai)
@@ -86,33 +133,32 @@ struct Walk {
         unsigned avail = ((1u << N) - 1u) & ~used;
         if constexpr (N - DEPTH == KB) {
             int bit[KB];
-#if HEGET_E_BY_PTR
-            using EA = const EEntry<T>*;
-#else
-            using EA = EEntry<T>;
-#endif
+            unsigned hb[KB];
+            // entries held in registers, or (HEGET_E_BY_PTR, and the lane-sharing fp64 kernels)
+            // pointers into the shared-memory table that are dereferenced at each use
+            constexpr bool BY_PTR = (HEGET_E_BY_PTR != 0) || (SHARE == 1 && HEGET_SHARE_BY_PTR != 0);
+            using EA = std::conditional_t<BY_PTR, const EEntry<T>*, EEntry<T>>;
             EA e[KB];
 #pragma unroll
             for (int m = 0; m < KB; ++m) {
                 const int i = __ffs(avail) - 1;
                 avail &= avail - 1u;
                 bit[m] = 1 << i;
-#if HEGET_E_BY_PTR
-                e[m] = &E[2 * i + ((hel >> i) & 1u)];
-#else
-                e[m] = E[2 * i + ((hel >> i) & 1u)];
-#endif
+                hb[m] = (hel >> i) & 1u;
+                if constexpr (BY_PTR)
+                    e[m] = &E[2 * i + hb[m]];
+                else
+                    e[m] = E[2 * i + hb[m]];
             }
-            Bottom<KB, T, EA>::run(P + used, bit, e, f, ar, ai);
+            Bottom<KB, T, EA, SHARE>::run(P + used, bit, e, hb, f, ar, ai);
         } else {
             while (avail) {
                 const int i = __ffs(avail) - 1;
                 avail &= avail - 1u;
                 const unsigned S = used | (1u << i);
                 const Spinor<T> fn = fvixx0_weyl(P[S], E[2 * i + ((hel >> i) & 1u)], f);
-                Walk<N, DEPTH + 1, KB, T>::run(P, E, hel, S, fn, ar, ai);
+                Walk<N, DEPTH + 1, KB, T, SHARE>::run(P, E, hel, S, fn, ar, ai);
             }
         }
     }
 };
-
