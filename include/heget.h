@@ -14,6 +14,8 @@
  *  - [dev] calls are asynchronous on `stream` (a cudaStream_t passed as void*, NULL = the
  *    legacy default stream) and do not synchronise the host; *_host calls return after
  *    the result is in the host buffer;
+ *  - a context is not thread-safe: calls on the SAME heget_ctx must not overlap in time
+ *    (different contexts, e.g. one per GPU or per host thread, are independent);
  *  - momenta layout: double[N][n+2][4], four-vectors (E,px,py,pz) (PAPER.md:474-477,
  *    553-554), particle order u, ubar, gamma_1..gamma_n (p1..p5 of List 2);
  *    the base pointer must be 16-byte aligned.
