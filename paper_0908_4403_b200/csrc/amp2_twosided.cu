@@ -183,11 +183,14 @@ struct TwoSidedSmem {
     static constexpr size_t bytes = off_list + (N + 1) * 72;
 };
 
+#ifndef HEGET_TS_MINB32
+#define HEGET_TS_MINB32 2   // 128 registers, two CTAs per SM: 6 gamma 9.8 -> 7.0 ms, 7 gamma 14.8 -> 12.5 ms
+#endif
 #ifndef HEGET_TS_MINB64
 #define HEGET_TS_MINB64 1
 #endif
 template <int N, typename T>
-__global__ void __launch_bounds__(Geometry<N>::THREADS, (sizeof(T) == 4) ? 1 : HEGET_TS_MINB64)
+__global__ void __launch_bounds__(Geometry<N>::THREADS, (sizeof(T) == 4) ? HEGET_TS_MINB32 : HEGET_TS_MINB64)
 amp2_twosided_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_t n_events, double g)
 {
     using G = Geometry<N>;
