@@ -1,0 +1,48 @@
+"""bench.py's reference arm (the CPU oracle on the host cores) runs without a GPU: its JSON line
+must carry the keys the driver's contract names, and the flop models bench.py reports must agree
+with the node counts of SURVEY 8(a)."""
+import json
+import math
+import os
+import subprocess
+import sys
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_reference_arm_prints_the_contract_line():
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--steps", "1",
+                          "--warmup", "0", "--config", "2gamma"], capture_output=True, text=True, timeout=600,
+                         env=dict(os.environ, RANK="0", WORLD_SIZE="1"))
+    assert out.returncode == 0, out.stderr
+    line = json.loads(out.stdout.strip().splitlines()[-1])
+    for key in ("impl", "metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better",
+                "scaling", "vs_baseline", "dtype", "data", "config", "cpu_baseline", "e2e"):
+        assert key in line, key
+    assert line["impl"] == "reference" and line["unit"] == "events/s" and line["value"] > 0
+    assert line["config"]["workload"] == "2gamma" and line["vs_baseline"] is None
+    assert line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["cores"] >= 1
+    assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["e2e"]["d2h_bytes_per_step"] == 0
+
+
+def test_other_ranks_of_the_reference_arm_exit_silently():
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--steps", "1",
+                          "--warmup", "0", "--config", "2gamma", "--gpus", "2"], capture_output=True, text=True,
+                         timeout=600, env=dict(os.environ, RANK="1", WORLD_SIZE="2"))
+    assert out.returncode == 0 and out.stdout.strip() == ""
+
+
+def test_flop_models_match_the_node_counts_of_the_survey():
+    sys.path.insert(0, ROOT)
+    import bench
+    internal = {2: 2, 3: 9, 4: 40, 5: 205, 6: 1236, 7: 8659, 8: 69280}
+    for n, nodes in internal.items():
+        assert bench.model_flops_per_event(n) == 2 * 2 ** n * (44 * nodes + 24 * math.factorial(n))
+        assert bench.executed_flops_per_event(n, "fp32") == 2 ** n * (36 * nodes + 10 * math.factorial(n))
+        assert bench.executed_flops_per_event(n, "fp64") <= bench.executed_flops_per_event(n, "fp32")
+        for algo in ("subset", "two-sided"):
+            assert 0 < bench.executed_flops_per_event_algo(n, algo) <= bench.executed_flops_per_event(n, "fp32") * 1.1
+    # model C as tabulated in SURVEY 8(d): 1.09e3, 7.5e4, 2.06e9 flop per event
+    assert abs(bench.model_flops_per_event(2) / 1.09e3 - 1) < 0.01
+    assert abs(bench.model_flops_per_event(4) / 7.5e4 - 1) < 0.01
+    assert abs(bench.model_flops_per_event(8) / 2.06e9 - 1) < 0.01
