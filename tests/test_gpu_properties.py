@@ -82,3 +82,20 @@ def test_algorithms_agree_on_every_event_of_the_headline_launch(hg):
         assert worst(hg.amp2(mom, FP64, algo=algo), t, passing) <= 2e-12
         assert worst(hg.amp2(mom, FP32, algo=algo), t, passing) <= 1e-4
     assert worst(hg.amp2(mom, FP32, algo=ALGO_TREE), t, passing) <= 1e-4
+
+
+@pytest.mark.parametrize("n,N", [(2, (1 << 18) + 37), (3, (1 << 19) + 37), (5, (1 << 18) + 5), (7, (1 << 13) + 1)])
+def test_three_organisations_of_the_sum_agree_on_large_ragged_batches(hg, n, N):
+    """The one-sided tree (with its helicity-lane sharing in fp64), two-sided chaining and the subset
+    recursion are three different evaluation orders of the same n! diagrams: on every event of a
+    large batch whose size is not a multiple of the events per CTA they must agree to rounding."""
+    for seed in (2, 3):
+        mom, w = hg.gen_events(seed, n, N, mode=workloads.LOGUNIFORM, a=100.0 * n, b=1500.0 * n, y_max=1.5,
+                               apply_cuts=True)
+        ok = w != 0
+        ref = hg.amp2(mom, FP64, algo=ALGO_SUBSET)
+        for algo in (ALGO_TREE, ALGO_TREE2):
+            for precision, tol in ((FP64, 2e-12), (FP32, 1e-4)):
+                got = hg.amp2(mom, precision, algo=algo)
+                assert torch.all(torch.isfinite(got)) and got.shape == (N,)
+                assert worst(got, ref, ok) <= tol
