@@ -421,7 +421,18 @@ def main():
         hg.histogram(mom_d, val, 0, 0.0, 1500.0, 60)
         ev[2].record()
         torch.cuda.synchronize()
-        result["next1"] = {"amp2_sampled_ms": ev[0].elapsed_time(ev[1]),
+        ev2 = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        hg.list2(cfg["seed"], mom_d, prec)
+        torch.cuda.synchronize()
+        ev2[0].record()
+        hg.list2(cfg["seed"], mom_d, prec)
+        ev2[1].record()
+        torch.cuda.synchronize()
+        result["next1"] = {"paper_list2_ms": ev2[0].elapsed_time(ev2[1]),
+                           "paper_list2_events_per_s": nl / (ev2[0].elapsed_time(ev2[1]) * 1e-3),
+                           "paper_list2_note": "heget_list2: the paper's List 2 program (thread per event, 4-component, "
+                                               "no reuse) on this GPU, same estimator as amp2_sampled",
+                           "amp2_sampled_ms": ev[0].elapsed_time(ev[1]),
                            "amp2_sampled_events_per_s": nl / (ev[0].elapsed_time(ev[1]) * 1e-3),
                            "histogram_ms": ev[1].elapsed_time(ev[2]), "events": nl, "precision": args.precision}
 

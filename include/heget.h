@@ -132,6 +132,15 @@ int heget_amp2_sampled(heget_ctx* ctx, uint64_t seed, uint64_t first_event, cons
                        int n, int precision, double* out_amp2, int32_t* out_hel, int64_t N,
                        void* stream);
 
+/* The paper's own program, List 2 generalised to n photons, run the way the
+ * paper runs it: one thread per event, one drawn helicity assignment per event, 4-component HEGET
+ * functions on cmplx w[6] (ixxxx1, oxxxx2, vxxxx0, n-1 fvoxx0 chained from the ubar line and one
+ * iovxxx per permutation, iPNext through the n! orderings), no prefix reuse, no tables.  Same
+ * arguments, helicity draw and result as heget_amp2_sampled (4 * 2^n * |M(h_e)|^2): it is the
+ * design this library is measured against on the same GPU. */
+int heget_list2(heget_ctx* ctx, uint64_t seed, uint64_t first_event, const double* momenta, int n,
+                int precision, double* out_amp2, int32_t* out_hel, int64_t N, void* stream);
+
 /* Kinematical distributions of Fig. 2 as weighted histograms, filled on the
  * device: event e adds value[e] (e.g. weight * amp2; 0 = event failed the cuts, skipped) at
  *   HEGET_OBS_PT_MAX  max_i pT(gamma_i)                         (eq. 9)

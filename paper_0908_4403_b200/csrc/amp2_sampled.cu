@@ -132,10 +132,82 @@ amp2_sampled_kernel(const double* __restrict__ momenta, uint64_t seed, uint64_t 
     }
 }
 
+// Small n: the whole event fits one THREAD (the paper's own mapping): its 2^N - 2
+// propagator entries and 2N polarisation entries live in thread-local arrays (L1-resident), the
+// tables are built with the same functions as everywhere else and the same Walk / Bottom code
+// walks the tree.  For small N a warp per event is mostly idle lanes in the table phase; measured
+// on B200 (2^20 events, fp64, warp -> thread per event): 2 gamma 0.54 -> 0.08 ms, 3 gamma 0.68 -> 0.11,
+// 4 gamma 0.78 -> 0.23, 5 gamma 1.28 -> 0.73; 6 gamma 4.5 -> 10.1 ms (the 62-entry table and the
+// deeper tree no longer fit the registers), so the switch is at N = 5.
+#ifndef HEGET_SAMPLED_THREAD_MAXN
+#define HEGET_SAMPLED_THREAD_MAXN 5
+#endif
+
+template <int N, typename T>
+__global__ void __launch_bounds__(128)
+amp2_sampled_thread_kernel(const double* __restrict__ momenta, uint64_t seed, uint64_t first_event,
+                           double* __restrict__ out, int32_t* __restrict__ out_hel, int64_t n_events, double g)
+{
+    constexpr int L = 1 << N;
+    constexpr int MOM = 4 * (N + 2);
+    const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n_events) return;
+    double mom[MOM];
+    {
+        const double2* src = reinterpret_cast<const double2*>(momenta + e * MOM);
+#pragma unroll
+        for (int k = 0; k < MOM / 2; ++k) {
+            const double2 v = src[k];
+            mom[2 * k] = v.x;
+            mom[2 * k + 1] = v.y;
+        }
+    }
+    const uint64_t gev = first_event + (uint64_t)e;
+    uint32_t x[4];
+    philox4x32_10((uint32_t)gev, (uint32_t)(gev >> 32), kHelicitySlot, 0u, (uint32_t)seed, (uint32_t)(seed >> 32), x);
+    const uint32_t bits = x[0] & ((1u << (N + 2)) - 1u);
+    const bool s1 = bits & 1u, s2 = (bits >> 1) & 1u;
+    double result = 0.0;
+    if (s1 != s2) {
+        const unsigned lam = (bits >> 2) & (unsigned)(L - 1);
+        const unsigned hel = s1 ? lam : (~lam & (unsigned)(L - 1));   // parity image for sigma_1 = -1
+        const double shat = 4.0 * mom[0] * mom[4];
+        const double scale = (sizeof(T) == 4) ? sqrt(shat) : 1.0;
+        PEntry<T> P[L];
+        EEntry<T> E[2 * N];
+        double fct = 4.0 * g * g * shat;
+#pragma unroll
+        for (int i = 0; i < N; ++i) fct *= make_photon_entries<T>(mom + 4 * (2 + i), &E[2 * i + 1], &E[2 * i]);
+#pragma unroll 1
+        for (unsigned S = 1; S <= (unsigned)(L - 2); ++S) {
+            if constexpr (sizeof(T) == 4)
+                make_subset_entry_plain<N>(mom, S, g, scale, &P[S]);
+            else
+                make_subset_entry<N, T>(mom, S, g, scale, &P[S]);
+        }
+        T ar = 0, ai = 0;
+        const Spinor<T> f0 = {(T)1, (T)0, (T)0, (T)0};
+        Walk<N, 0, N, T>::run(P, E, hel, 0u, f0, ar, ai);
+        if (sizeof(T) == 4) {
+            const double inv = 1.0 / shat;
+#pragma unroll
+            for (int i = 0; i < N - 1; ++i) fct *= inv;
+        }
+        result = fct * ((double)ar * (double)ar + (double)ai * (double)ai);
+    }
+    out[e] = result;
+    if (out_hel) out_hel[e] = (int32_t)bits;
+}
+
 template <int N, typename T>
 cudaError_t launch_one(const double* momenta, uint64_t seed, uint64_t first_event, double* out, int32_t* out_hel,
                        int64_t n_events, double g, cudaStream_t stream)
 {
+    if constexpr (N <= HEGET_SAMPLED_THREAD_MAXN) {
+        amp2_sampled_thread_kernel<N, T><<<(unsigned)((n_events + 127) / 128), 128, 0, stream>>>(
+            momenta, seed, first_event, out, out_hel, n_events, g);
+        return cudaGetLastError();
+    }
     const int64_t blocks = (n_events + kWarpsPerCta<N> - 1) / kWarpsPerCta<N>;
     amp2_sampled_kernel<N, T><<<(unsigned)blocks, kWarpsPerCta<N> * 32, 0, stream>>>(momenta, seed, first_event, out,
                                                                                   out_hel, n_events, g);

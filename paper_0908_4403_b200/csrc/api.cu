@@ -180,6 +180,20 @@ int heget_amp2_sampled(heget_ctx* ctx, uint64_t seed, uint64_t first_event, cons
     return err == cudaSuccess ? HEGET_OK : fail_cuda(ctx, err);
 }
 
+int heget_list2(heget_ctx* ctx, uint64_t seed, uint64_t first_event, const double* momenta, int n, int precision,
+                double* out_amp2, int32_t* out_hel, int64_t N, void* stream)
+{
+    if (!ctx || n < 2 || n > 8 || N < 0 || (N > 0 && (!momenta || !out_amp2))) return HEGET_EINVAL;
+    if (precision != HEGET_FP32 && precision != HEGET_FP64) return HEGET_EINVAL;
+    DeviceGuard guard(ctx->device);
+    if (!guard.ok) return fail_cuda(ctx, cudaGetLastError());
+    int launches = 0;
+    cudaError_t err = heget_launch_list2(ctx, seed, first_event, momenta, n, precision, out_amp2, out_hel, N,
+                                         (cudaStream_t)stream, &launches);
+    ctx->launches += launches;
+    return err == cudaSuccess ? HEGET_OK : fail_cuda(ctx, err);
+}
+
 int heget_histogram(heget_ctx* ctx, const double* momenta, const double* value, int n, int64_t N, int observable,
                     double lo, double hi, int nbins, double* hist, void* stream)
 {
