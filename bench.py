@@ -428,6 +428,23 @@ def main():
         hg.list2(cfg["seed"], mom_d, prec)
         ev2[1].record()
         torch.cuda.synchronize()
+        # the paper's arithmetic for the headline quantity on this GPU: List 2 called for all 4*2^n
+        # helicity assignments per thread (model A of SURVEY 8(d)); bounded to n <= 6
+        if n <= 6:
+            n_pd = nl if n <= 4 else nl // 64
+            ev3 = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+            sub = mom_d[:n_pd].contiguous()
+            hg.list2_sum(sub, prec)
+            torch.cuda.synchronize()
+            ev3[0].record()
+            hg.list2_sum(sub, prec)
+            ev3[1].record()
+            torch.cuda.synchronize()
+            pd_ms = ev3[0].elapsed_time(ev3[1])
+            result["paper_design"] = {"events_per_s": n_pd / (pd_ms * 1e-3), "ms": pd_ms, "events": n_pd,
+                                      "note": "heget_list2_sum: the paper's List 2 program (thread per event, "
+                                              "4-component, no prefix reuse, no parity) looped over all helicity "
+                                              "assignments, same GPU, same precision, same momenta"}
         result["next1"] = {"paper_list2_ms": ev2[0].elapsed_time(ev2[1]),
                            "paper_list2_events_per_s": nl / (ev2[0].elapsed_time(ev2[1]) * 1e-3),
                            "paper_list2_note": "heget_list2: the paper's List 2 program (thread per event, 4-component, "

@@ -141,6 +141,13 @@ int heget_amp2_sampled(heget_ctx* ctx, uint64_t seed, uint64_t first_event, cons
 int heget_list2(heget_ctx* ctx, uint64_t seed, uint64_t first_event, const double* momenta, int n,
                 int precision, double* out_amp2, int32_t* out_hel, int64_t N, void* stream);
 
+/* The same program called for every one of the 4 * 2^n helicity assignments inside the thread:
+ * out_amp2[e] = sum |M|^2, the quantity heget_amp2 returns, computed with the paper's arithmetic
+ * (no prefix reuse, no parity, 4-component; SURVEY 8(d) model A).  A same-GPU baseline for the
+ * headline metric; n = 7, 8 take minutes per 10^4 events. */
+int heget_list2_sum(heget_ctx* ctx, const double* momenta, int n, int precision, double* out_amp2,
+                    int64_t N, void* stream);
+
 /* Kinematical distributions of Fig. 2 as weighted histograms, filled on the
  * device: event e adds value[e] (e.g. weight * amp2; 0 = event failed the cuts, skipped) at
  *   HEGET_OBS_PT_MAX  max_i pT(gamma_i)                         (eq. 9)

@@ -19,7 +19,7 @@ VTX_IOVXXX, VTX_FVIXX0, VTX_FVOXX0, VTX_JIOXX0 = range(4)
 GEN_FIXED, GEN_LOGUNIFORM, GEN_TOYPDF = 0, 1, 2
 
 EXPORTS = ["heget_init", "heget_destroy", "heget_strerror", "heget_last_cuda_error", "heget_rambo",
-           "heget_gen_events", "heget_amp2", "heget_amp2_algo", "heget_amp2_sampled", "heget_list2", "heget_histogram", "heget_helas_wavefunction", "heget_helas_vertex", "heget_xsec_reduce", "heget_xsec_host", "heget_fma_peak", "heget_fma_peak_pattern",
+           "heget_gen_events", "heget_amp2", "heget_amp2_algo", "heget_amp2_sampled", "heget_list2", "heget_list2_sum", "heget_histogram", "heget_helas_wavefunction", "heget_helas_vertex", "heget_xsec_reduce", "heget_xsec_host", "heget_fma_peak", "heget_fma_peak_pattern",
            "heget_launch_count"]
 
 
@@ -66,6 +66,8 @@ def load_library():
     lib.heget_amp2_sampled.restype = ci
     lib.heget_list2.argtypes = [vp, u64, u64, dp, ci, ci, dp, vp, i64, vp]
     lib.heget_list2.restype = ci
+    lib.heget_list2_sum.argtypes = [vp, dp, ci, ci, dp, i64, vp]
+    lib.heget_list2_sum.restype = ci
     lib.heget_histogram.argtypes = [vp, dp, dp, ci, i64, ci, cd, cd, ci, dp, vp]
     lib.heget_histogram.restype = ci
     lib.heget_helas_wavefunction.argtypes = [vp, ci, ci, dp, ci, ci, dp, i64, vp]
@@ -185,6 +187,15 @@ class Heget:
                                           out.data_ptr(), out_hel.data_ptr(), N, _stream_ptr(self.device)),
                     "heget_list2")
         return out, out_hel
+
+    def list2_sum(self, momenta, precision=FP64):
+        """The paper's List 2 program looped over all helicity assignments: same result as amp2."""
+        _check_dev(momenta, None, self.device)
+        N, n = momenta.shape[0], momenta.shape[1] - 2
+        out = torch.empty((N,), dtype=torch.float64, device=self.device)
+        self._check(self._lib.heget_list2_sum(self._ctx, momenta.data_ptr(), n, precision, out.data_ptr(), N,
+                                              _stream_ptr(self.device)), "heget_list2_sum")
+        return out
 
     def histogram(self, momenta, value, observable, lo, hi, nbins, hist=None):
         """Weighted histogram [underflow, nbins bins, overflow] of max pT / min Delta R / all Delta R."""

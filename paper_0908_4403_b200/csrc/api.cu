@@ -188,7 +188,21 @@ int heget_list2(heget_ctx* ctx, uint64_t seed, uint64_t first_event, const doubl
     DeviceGuard guard(ctx->device);
     if (!guard.ok) return fail_cuda(ctx, cudaGetLastError());
     int launches = 0;
-    cudaError_t err = heget_launch_list2(ctx, seed, first_event, momenta, n, precision, out_amp2, out_hel, N,
+    cudaError_t err = heget_launch_list2(ctx, seed, first_event, momenta, n, precision, out_amp2, out_hel, N, false,
+                                         (cudaStream_t)stream, &launches);
+    ctx->launches += launches;
+    return err == cudaSuccess ? HEGET_OK : fail_cuda(ctx, err);
+}
+
+int heget_list2_sum(heget_ctx* ctx, const double* momenta, int n, int precision, double* out_amp2, int64_t N,
+                    void* stream)
+{
+    if (!ctx || n < 2 || n > 8 || N < 0 || (N > 0 && (!momenta || !out_amp2))) return HEGET_EINVAL;
+    if (precision != HEGET_FP32 && precision != HEGET_FP64) return HEGET_EINVAL;
+    DeviceGuard guard(ctx->device);
+    if (!guard.ok) return fail_cuda(ctx, cudaGetLastError());
+    int launches = 0;
+    cudaError_t err = heget_launch_list2(ctx, 0, 0, momenta, n, precision, out_amp2, nullptr, N, true,
                                          (cudaStream_t)stream, &launches);
     ctx->launches += launches;
     return err == cudaSuccess ? HEGET_OK : fail_cuda(ctx, err);

@@ -42,7 +42,7 @@ cudaError_t heget_launch_amp2_sampled(const heget_ctx* ctx, uint64_t seed, uint6
                                       const double* momenta, int n, int precision, double* out_amp2,
                                       int32_t* out_hel, int64_t N, cudaStream_t stream, int* launches);
 cudaError_t heget_launch_list2(const heget_ctx* ctx, uint64_t seed, uint64_t first_event, const double* momenta,
-                               int n, int precision, double* out_amp2, int32_t* out_hel, int64_t N,
+                               int n, int precision, double* out_amp2, int32_t* out_hel, int64_t N, bool sum,
                                cudaStream_t stream, int* launches);
 cudaError_t heget_launch_histogram(const heget_ctx* ctx, const double* momenta, const double* value, int n,
                                    int64_t N, int observable, double lo, double hi, int nbins, double* hist,

@@ -35,34 +35,19 @@ __device__ __forceinline__ bool ipnext(int* a)
     return true;
 }
 
+// List 2 for one event and one helicity assignment `bits` (bit k: particle k in the order u,
+// ubar, gamma_1..gamma_n; 1 -> +1): returns |ampsum|^2 in the units of p.
 template <int N, typename T>
-__global__ void __launch_bounds__(256)
-list2_kernel(const double* __restrict__ momenta, uint64_t seed, uint64_t first_event, double* __restrict__ out,
-             int32_t* __restrict__ out_hel, int64_t n_events, double g)
+__device__ __forceinline__ double list2_program(const T (&p)[N + 2][4], uint32_t bits, T gau)
 {
-    const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= n_events) return;
-    const double* mom = momenta + e * 4 * (N + 2);
-    const double shat = 4.0 * mom[0] * mom[4];
-    const double unit = (sizeof(T) == 4) ? 1.0 / sqrt(shat) : 1.0;
-
-    uint32_t x[4];
-    const uint64_t gev = first_event + (uint64_t)e;
-    philox4x32_10((uint32_t)gev, (uint32_t)(gev >> 32), kHelicitySlot, 0u, (uint32_t)seed, (uint32_t)(seed >> 32), x);
-    const uint32_t bits = x[0] & ((1u << (N + 2)) - 1u);
-
     cmplx<T> w[N + 2][6];
 #pragma unroll
     for (int k = 0; k < N + 2; ++k) {
-        const T p[4] = {(T)(mom[4 * k] * unit), (T)(mom[4 * k + 1] * unit), (T)(mom[4 * k + 2] * unit),
-                        (T)(mom[4 * k + 3] * unit)};
         const int nh = ((bits >> k) & 1u) ? +1 : -1;
-        if (k == 0) ixxxx1(p, nh, +1, w[0]);
-        else if (k == 1) oxxxx2(p, nh, -1, w[1]);
-        else vxxxx0(p, nh, +1, w[k]);
+        if (k == 0) ixxxx1(p[0], nh, +1, w[0]);
+        else if (k == 1) oxxxx2(p[1], nh, -1, w[1]);
+        else vxxxx0(p[k], nh, +1, w[k]);
     }
-
-    const T gau = (T)g;
     cmplx<T> ampsum = mkcmplx((T)0, (T)0);
     int a[N];
 #pragma unroll
@@ -78,8 +63,40 @@ list2_kernel(const double* __restrict__ momenta, uint64_t seed, uint64_t first_e
         }
         ampsum = ampsum + iovxxx(w[0], wa, w[a[N - 1]], gau);
     } while (ipnext<N>(a));
+    return (double)ampsum.re * (double)ampsum.re + (double)ampsum.im * (double)ampsum.im;
+}
 
-    double r = 4.0 * (double)(1 << N) * ((double)ampsum.re * (double)ampsum.re + (double)ampsum.im * (double)ampsum.im);
+// SUM = false: one drawn helicity assignment per event (the paper's loop), out = 4 2^n |M(h)|^2.
+// SUM = true: the same program called for every one of the 4 2^n assignments, out = sum |M|^2 --
+// the paper's arithmetic (SURVEY 8(d) model A) for the quantity heget_amp2 returns.
+template <int N, typename T, bool SUM>
+__global__ void __launch_bounds__(256)
+list2_kernel(const double* __restrict__ momenta, uint64_t seed, uint64_t first_event, double* __restrict__ out,
+             int32_t* __restrict__ out_hel, int64_t n_events, double g)
+{
+    const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n_events) return;
+    const double* mom = momenta + e * 4 * (N + 2);
+    const double shat = 4.0 * mom[0] * mom[4];
+    const double unit = (sizeof(T) == 4) ? 1.0 / sqrt(shat) : 1.0;
+    T p[N + 2][4];
+#pragma unroll
+    for (int k = 0; k < N + 2; ++k)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) p[k][c] = (T)(mom[4 * k + c] * unit);
+
+    double r;
+    uint32_t bits = 0u;
+    if constexpr (SUM) {
+        r = 0.0;
+        for (uint32_t h = 0; h < (4u << N); ++h) r += list2_program<N, T>(p, h, (T)g);
+    } else {
+        uint32_t x[4];
+        const uint64_t gev = first_event + (uint64_t)e;
+        philox4x32_10((uint32_t)gev, (uint32_t)(gev >> 32), kHelicitySlot, 0u, (uint32_t)seed, (uint32_t)(seed >> 32), x);
+        bits = x[0] & ((1u << (N + 2)) - 1u);
+        r = 4.0 * (double)(1 << N) * list2_program<N, T>(p, bits, (T)g);
+    }
     if (sizeof(T) == 4) {
         // amplitude ~ (energy)^(2-n): |M|^2 in units of sqrt(s_hat) times s_hat^(2-n)
         const double inv = 1.0 / shat;
@@ -87,30 +104,33 @@ list2_kernel(const double* __restrict__ momenta, uint64_t seed, uint64_t first_e
         for (int i = 0; i < N - 2; ++i) r *= inv;
     }
     out[e] = r;
-    if (out_hel) out_hel[e] = (int32_t)bits;
+    if (!SUM && out_hel) out_hel[e] = (int32_t)bits;
 }
 
 template <int N, typename T>
 cudaError_t launch_one(const double* momenta, uint64_t seed, uint64_t first_event, double* out, int32_t* out_hel,
-                       int64_t n_events, double g, cudaStream_t stream)
+                       int64_t n_events, double g, bool sum, cudaStream_t stream)
 {
     const int64_t blocks = (n_events + 255) / 256;
-    list2_kernel<N, T><<<(unsigned)blocks, 256, 0, stream>>>(momenta, seed, first_event, out, out_hel, n_events, g);
+    if (sum)
+        list2_kernel<N, T, true><<<(unsigned)blocks, 256, 0, stream>>>(momenta, seed, first_event, out, out_hel, n_events, g);
+    else
+        list2_kernel<N, T, false><<<(unsigned)blocks, 256, 0, stream>>>(momenta, seed, first_event, out, out_hel, n_events, g);
     return cudaGetLastError();
 }
 
 template <typename T>
 cudaError_t launch_n(int n, const double* momenta, uint64_t seed, uint64_t first_event, double* out,
-                     int32_t* out_hel, int64_t n_events, double g, cudaStream_t stream)
+                     int32_t* out_hel, int64_t n_events, double g, bool sum, cudaStream_t stream)
 {
     switch (n) {
-        case 2: return launch_one<2, T>(momenta, seed, first_event, out, out_hel, n_events, g, stream);
-        case 3: return launch_one<3, T>(momenta, seed, first_event, out, out_hel, n_events, g, stream);
-        case 4: return launch_one<4, T>(momenta, seed, first_event, out, out_hel, n_events, g, stream);
-        case 5: return launch_one<5, T>(momenta, seed, first_event, out, out_hel, n_events, g, stream);
-        case 6: return launch_one<6, T>(momenta, seed, first_event, out, out_hel, n_events, g, stream);
-        case 7: return launch_one<7, T>(momenta, seed, first_event, out, out_hel, n_events, g, stream);
-        case 8: return launch_one<8, T>(momenta, seed, first_event, out, out_hel, n_events, g, stream);
+        case 2: return launch_one<2, T>(momenta, seed, first_event, out, out_hel, n_events, g, sum, stream);
+        case 3: return launch_one<3, T>(momenta, seed, first_event, out, out_hel, n_events, g, sum, stream);
+        case 4: return launch_one<4, T>(momenta, seed, first_event, out, out_hel, n_events, g, sum, stream);
+        case 5: return launch_one<5, T>(momenta, seed, first_event, out, out_hel, n_events, g, sum, stream);
+        case 6: return launch_one<6, T>(momenta, seed, first_event, out, out_hel, n_events, g, sum, stream);
+        case 7: return launch_one<7, T>(momenta, seed, first_event, out, out_hel, n_events, g, sum, stream);
+        case 8: return launch_one<8, T>(momenta, seed, first_event, out, out_hel, n_events, g, sum, stream);
         default: return cudaErrorInvalidValue;
     }
 }
@@ -118,13 +138,13 @@ cudaError_t launch_n(int n, const double* momenta, uint64_t seed, uint64_t first
 }  // namespace
 
 cudaError_t heget_launch_list2(const heget_ctx* ctx, uint64_t seed, uint64_t first_event, const double* momenta,
-                               int n, int precision, double* out_amp2, int32_t* out_hel, int64_t N,
+                               int n, int precision, double* out_amp2, int32_t* out_hel, int64_t N, bool sum,
                                cudaStream_t stream, int* launches)
 {
     *launches = 0;
     if (N == 0) return cudaSuccess;
     *launches = 1;
     if (precision == HEGET_FP32)
-        return launch_n<float>(n, momenta, seed, first_event, out_amp2, out_hel, N, ctx->g, stream);
-    return launch_n<double>(n, momenta, seed, first_event, out_amp2, out_hel, N, ctx->g, stream);
+        return launch_n<float>(n, momenta, seed, first_event, out_amp2, out_hel, N, ctx->g, sum, stream);
+    return launch_n<double>(n, momenta, seed, first_event, out_amp2, out_hel, N, ctx->g, sum, stream);
 }

@@ -192,3 +192,23 @@ def test_paper_list2_program_matches_oracle_and_the_sampled_kernel(hg, n, precis
           % (n, "fp64" if precision == FP64 else "fp32", N, err[passing].max(), np.median(err[passing]), err.max()))
     assert np.all(err[passing] <= tol) and np.all(err <= tol * 1e3)
     assert np.all(np.abs(got - ours)[passing] <= 2 * tol * scale[passing])
+
+
+@pytest.mark.parametrize("n", [2, 3, 4, 5])
+@pytest.mark.parametrize("precision", [FP64, FP32])
+def test_paper_list2_summed_over_helicities_matches_oracle_and_heget_amp2(hg, n, precision):
+    """heget_list2_sum: the paper's program called for all 4*2^n helicity assignments (the paper's
+    arithmetic for the north-star quantity).  Same accuracy class as heget_list2 (plain p_f^2)."""
+    N = {2: 700, 3: 400, 4: 300, 5: 100}[n]
+    mom, w = events(n, N)
+    ref = oracle.amp2(mom, extended=True)
+    d = torch.from_numpy(mom).cuda()
+    got = hg.list2_sum(d, precision).cpu().numpy()
+    ours = hg.amp2(d, precision).cpu().numpy()
+    tol = 1e-10 if precision == FP64 else 2e-3
+    passing = w != 0
+    err = np.abs(got / ref - 1.0)
+    print("\n[list2 sum parity] n=%d %s events=%d: passing max %.3e median %.3e, all max %.3e"
+          % (n, "fp64" if precision == FP64 else "fp32", N, err[passing].max(), np.median(err[passing]), err.max()))
+    assert np.all(err[passing] <= tol) and np.all(err <= tol * 1e3)
+    assert np.all(np.abs(got / ours - 1.0)[passing] <= 2 * tol)
