@@ -361,6 +361,10 @@ def main():
                 "peak_three_register_fma": peak_3reg / 1e12, "peak_node_pattern": peak_node / 1e12,
                 "frac_of_node_pattern": achieved / peak_node,
                 "model_c_tflops": model_c / 1e12, "model_c_frac": model_c / peak_measured,
+                "frac_note": "frac counts EXECUTED flops (what ncu counts); model_c_frac counts SURVEY 8(d)'s fixed "
+                             "algorithmic figure (model C) over the same time.  Work removed by the parity relation and "
+                             "by sharing spinors between helicity lanes lowers frac while events/s and model_c_frac "
+                             "rise (4 gamma fp64: v3 1.48 ms, frac 0.56 -> v4 1.19 ms, frac 0.37)",
                 "flops_model": "executed: 2^n lanes x (36 flop per tree node + 10 per leaf), minus the nodes the fp64 "
                                "kernels share between helicity lanes (see executed_flops_per_event); model C (SURVEY "
                                "8(d)): 2*2^n x (44 per node + 24 per leaf), 2.5-5x the executed count because the kernel "
