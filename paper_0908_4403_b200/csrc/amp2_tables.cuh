@@ -103,10 +103,14 @@ __device__ __forceinline__ void make_subset_entry(const double* mom, unsigned S,
 {
     const double e1 = mom[0];
     dd pe = {e1, 0.0}, pz = {mom[3], 0.0}, px = {mom[1], 0.0}, py = {mom[2], 0.0};
+    // a proper subset has at most N-1 members: N-1 rounds over "the next member of S" instead of
+    // N rounds over all photons (lanes with fewer members idle in the last rounds)
+    unsigned rem = S;
 #pragma unroll
-    for (int i = 0; i < N; ++i) {
-        if ((S >> i) & 1u) {
-            const double* k = mom + 4 * (2 + i);
+    for (int j = 0; j < N - 1; ++j) {
+        if (rem) {
+            const double* k = mom + 4 * (2 + (__ffs(rem) - 1));
+            rem &= rem - 1u;
             dd_acc(pe, -k[0]);
             dd_acc(px, -k[1]);
             dd_acc(py, -k[2]);
