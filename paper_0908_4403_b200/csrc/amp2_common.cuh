@@ -6,6 +6,10 @@
 #include "amp2_tables.cuh"
 #include "heget_internal.cuh"
 
+#ifndef HEGET_UNIFORM_TABLES
+#define HEGET_UNIFORM_TABLES 1
+#endif
+
 template <typename T>
 struct alignas(16) Spinor {
     T r0, i0, r1, i1;  // two complex components
@@ -67,14 +71,35 @@ __device__ __forceinline__ void build_tables(double g, const double* s_mom, PEnt
     const double* mom = s_mom + ev_local * MOM;
     const double shat = 4.0 * mom[0] * mom[4];  // (p1+p2)^2 for p1 || +z, p2 || -z
     const double scale = (sizeof(T) == 4) ? sqrt(shat) : 1.0;
-    if (hel < (unsigned)N)
-        s_s2[ev_local * N + hel] = make_photon_entries<T>(mom + 4 * (2 + hel), &s_E[(ev_local * N + hel) * 2 + 1],
-                                                          &s_E[(ev_local * N + hel) * 2 + 0]);
-    if (hel >= 1u && hel <= (unsigned)(G::L - 2)) {
+    if constexpr (HEGET_UNIFORM_TABLES != 0 && N >= 4) {  // measured: 4 gamma fp64 -2.5 %, 3 gamma +12 %
+        // branch-free form: every lane evaluates a photon (its own, or the last one) and a subset
+        // (its own, or the nearest proper one) in ONE instruction stream -- no reconvergence points,
+        // and the two independent dependency chains interleave; only the stores are predicated
+        const unsigned ph = hel < (unsigned)N ? hel : (unsigned)(N - 1);
+        const unsigned S = hel < 1u ? 1u : (hel > (unsigned)(G::L - 2) ? (unsigned)(G::L - 2) : hel);
+        EEntry<T> ep, em;
+        PEntry<T> pe;
+        const double s2 = make_photon_entries<T>(mom + 4 * (2 + ph), &ep, &em);
         if constexpr (sizeof(T) == 4)
-            make_subset_entry_plain<N>(mom, hel, g, scale, &s_P[ev_local * G::L + hel]);
+            make_subset_entry_plain<N>(mom, S, g, scale, &pe);
         else
-            make_subset_entry<N, T>(mom, hel, g, scale, &s_P[ev_local * G::L + hel]);
+            make_subset_entry<N, T>(mom, S, g, scale, &pe);
+        if (hel < (unsigned)N) {
+            s_s2[ev_local * N + hel] = s2;
+            s_E[(ev_local * N + hel) * 2 + 1] = ep;
+            s_E[(ev_local * N + hel) * 2 + 0] = em;
+        }
+        if (S == hel) s_P[ev_local * G::L + hel] = pe;
+    } else {
+        if (hel < (unsigned)N)
+            s_s2[ev_local * N + hel] = make_photon_entries<T>(mom + 4 * (2 + hel), &s_E[(ev_local * N + hel) * 2 + 1],
+                                                              &s_E[(ev_local * N + hel) * 2 + 0]);
+        if (hel >= 1u && hel <= (unsigned)(G::L - 2)) {
+            if constexpr (sizeof(T) == 4)
+                make_subset_entry_plain<N>(mom, hel, g, scale, &s_P[ev_local * G::L + hel]);
+            else
+                make_subset_entry<N, T>(mom, hel, g, scale, &s_P[ev_local * G::L + hel]);
+        }
     }
     __syncthreads();
 }
