@@ -101,13 +101,18 @@ template <int N, typename T>
 __device__ __forceinline__ void make_subset_entry(const double* mom, unsigned S, double g, double scale,
                                                   PEntry<T>* out)
 {
-    const double e1 = mom[0];
-    dd pe = {e1, 0.0}, pz = {mom[3], 0.0}, px = {mom[1], 0.0}, py = {mom[2], 0.0};
-    // a proper subset has at most N-1 members: N-1 rounds over "the next member of S" instead of
-    // N rounds over all photons (lanes with fewer members idle in the last rounds)
+    // p1 = (E1, 0, 0, E1) (precondition of include/heget.h): the transverse sums start from the
+    // first member exactly, the others from p1.  A proper subset has 1..N-1 members: one
+    // unconditional round and N-2 rounds over "the next member of S" instead of N rounds over all
+    // photons (lanes with fewer members idle in the last rounds).
     unsigned rem = S;
+    const double* k0 = mom + 4 * (2 + (__ffs(rem) - 1));
+    rem &= rem - 1u;
+    dd pe = {mom[0], 0.0}, pz = {mom[3], 0.0}, px = {-k0[1], 0.0}, py = {-k0[2], 0.0};
+    dd_acc(pe, -k0[0]);
+    dd_acc(pz, -k0[3]);
 #pragma unroll
-    for (int j = 0; j < N - 1; ++j) {
+    for (int j = 1; j < N - 1; ++j) {
         if (rem) {
             const double* k = mom + 4 * (2 + (__ffs(rem) - 1));
             rem &= rem - 1u;
