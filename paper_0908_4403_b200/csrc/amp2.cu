@@ -20,6 +20,17 @@
 #define HEGET_MINB64 2
 #endif
 
+// CTA size of the tree kernels.  Small CTAs (64 threads: 4 events at n = 4) put more CTAs, each in
+// its own phase (load / tables / tree), on an SM at the same number of warps, which overlaps the
+// latency-bound phases better: measured on B200, 256 -> 64 threads: 4 gamma fp64 1.114 -> 1.012 ms,
+// fp32 0.748 -> 0.731 ms, 3 gamma fp64 0.256 -> 0.238 ms, 5-7 gamma 1-2 %.  (The subset and two-sided
+// kernels keep 256: they copy index tables per CTA and lose up to 2x at 64.)
+#ifndef HEGET_TREE_CTA_THREADS
+#define HEGET_TREE_CTA_THREADS 64
+#endif
+template <int N>
+using TreeGeometry = Geometry<N, HEGET_TREE_CTA_THREADS>;
+
 namespace {
 
 #ifndef HEGET_SHARE32_MAXN
@@ -52,16 +63,20 @@ constexpr int kBottom = (N < HEGET_KB) ? N : HEGET_KB;  // unrolled bottom level
 // 0.862 -> 0.755 ms, 5 gamma 6.48 -> 6.39 ms; fp32 3 gamma and every fp64 kernel are 1-6 % SLOWER
 // that way (two 128-register CTAs per SM overlap their phases better when CTAs turn over), so
 // those keep one batch per CTA.
+#ifndef HEGET_PERSIST64_N4
+#define HEGET_PERSIST64_N4 0
+#endif
 template <int N, typename T>
-constexpr bool kPersistent = (sizeof(T) == 4) && (N == 4 || N == 5);
+constexpr bool kPersistent = ((sizeof(T) == 4) && (N == 4 || N == 5)) || (HEGET_PERSIST64_N4 != 0 && sizeof(T) == 8 && N == 4);
 
 template <int N, typename T>
-__global__ void __launch_bounds__(Geometry<N>::THREADS, (sizeof(T) == 4) ? HEGET_MINB32 : HEGET_MINB64)
+__global__ void __launch_bounds__(TreeGeometry<N>::THREADS,
+                                  ((sizeof(T) == 4) ? HEGET_MINB32 : HEGET_MINB64) * 256 / TreeGeometry<N>::THREADS)
 amp2_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_t n_events, double g,
             int64_t n_batches)
 {
-    using G = Geometry<N>;
-    using Tile = MomentaTile<N>;
+    using G = TreeGeometry<N>;
+    using Tile = MomentaTile<N, G>;
     constexpr int MOM = 4 * (N + 2);
     __shared__ __align__(16) double s_mom[G::EPB * MOM];
     __shared__ PEntry<T> s_P[G::EPB * G::L];
@@ -83,7 +98,7 @@ amp2_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_
         if constexpr (kPersistent<N, T>) {
             if (batch + gridDim.x < n_batches) Tile::load(momenta, (batch + gridDim.x) * G::EPB, n_events, pf);
         }
-        build_tables<N, T>(g, s_mom, s_P, s_E, s_s2);                        // a4, a5 (ends with a barrier)
+        build_tables<N, T, G>(g, s_mom, s_P, s_E, s_s2);                        // a4, a5 (ends with a barrier)
 
         // a2, a6, a7: psi_0 = u(p1,+)/sqrt(2E1) = (1,0); walk the permutation tree
         T ar = 0, ai = 0;
@@ -112,7 +127,7 @@ amp2_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_
         }
 
         // a8: |ampsum|^2 summed over the event's 2^N lanes, constant factors, store
-        finish_event<N, T>(ar, ai, s_mom, s_s2, s_red, g, out, batch * G::EPB, n_events);
+        finish_event<N, T, G>(ar, ai, s_mom, s_s2, s_red, g, out, batch * G::EPB, n_events);
         if constexpr (kPersistent<N, T>) __syncthreads();                    // tables are rewritten next round
     } while (kPersistent<N, T> && (batch += gridDim.x) < n_batches);
 }
@@ -121,7 +136,7 @@ template <int N, typename T>
 cudaError_t launch_one(const heget_ctx* ctx, const double* momenta, double* out, int64_t n_events, double g,
                        cudaStream_t stream)
 {
-    using G = Geometry<N>;
+    using G = TreeGeometry<N>;
     const int64_t n_batches = (n_events + G::EPB - 1) / G::EPB;
     int64_t blocks = n_batches;
     if (kPersistent<N, T>) {

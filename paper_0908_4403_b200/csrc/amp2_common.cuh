@@ -6,6 +6,9 @@
 #include "amp2_tables.cuh"
 #include "heget_internal.cuh"
 
+#ifndef HEGET_CTA_THREADS
+#define HEGET_CTA_THREADS 256   // default CTA size (at least one event's 2^N lanes)
+#endif
 #ifndef HEGET_UNIFORM_TABLES
 #define HEGET_UNIFORM_TABLES 1
 #endif
@@ -15,20 +18,20 @@ struct alignas(16) Spinor {
     T r0, i0, r1, i1;  // two complex components
 };
 
-// One lane per photon-helicity configuration: 2^N lanes per event, 256-thread CTAs.
-template <int N>
+// One lane per photon-helicity configuration: 2^N lanes per event, CTAs of CTA threads (or one
+// event's lanes if that is more).
+template <int N, int CTA = HEGET_CTA_THREADS>
 struct Geometry {
     static constexpr int L = 1 << N;                       // lanes (helicity configurations) per event
-    static constexpr int THREADS = (L > 256) ? L : 256;
+    static constexpr int THREADS = (L > CTA) ? L : CTA;
     static constexpr int EPB = THREADS / L;                // events per CTA
 };
 
 // a1: the CTA's momenta as double2 words, PF words per thread: global -> registers
 // (events past the end re-read the last event) and registers -> shared memory.  Split in two
 // so that a persistent CTA can have the next batch's loads in flight while it computes.
-template <int N>
+template <int N, typename G = Geometry<N>>
 struct MomentaTile {
-    using G = Geometry<N>;
     static constexpr int MOM = 4 * (N + 2);
     static constexpr int WORDS = G::EPB * MOM / 2;
     static constexpr int PF = (WORDS + G::THREADS - 1) / G::THREADS;
@@ -60,11 +63,10 @@ struct MomentaTile {
 
 // a4: vxxxx0 for both helicities of photon `hel` (lanes 0..N-1 of each event);
 // a5: subset kinematics, one subset per lane.  Reads s_mom (barrier before), ends with a barrier.
-template <int N, typename T>
+template <int N, typename T, typename G = Geometry<N>>
 __device__ __forceinline__ void build_tables(double g, const double* s_mom, PEntry<T>* s_P, EEntry<T>* s_E,
                                              double* s_s2)
 {
-    using G = Geometry<N>;
     constexpr int MOM = 4 * (N + 2);
     const int ev_local = threadIdx.x / G::L;
     const unsigned hel = threadIdx.x % G::L;
@@ -105,25 +107,24 @@ __device__ __forceinline__ void build_tables(double g, const double* s_mom, PEnt
 }
 
 // a1 + a4 + a5 for the batch of events starting at ev0 (one-shot form).
-template <int N, typename T>
+template <int N, typename T, typename G = Geometry<N>>
 __device__ __forceinline__ void build_event_tables(const double* __restrict__ momenta, int64_t ev0, int64_t n_events,
                                                    double g, double* s_mom, PEntry<T>* s_P, EEntry<T>* s_E,
                                                    double* s_s2)
 {
-    double2 r[MomentaTile<N>::PF];
-    MomentaTile<N>::load(momenta, ev0, n_events, r);
-    MomentaTile<N>::store(s_mom, r);
+    double2 r[MomentaTile<N, G>::PF];
+    MomentaTile<N, G>::load(momenta, ev0, n_events, r);
+    MomentaTile<N, G>::store(s_mom, r);
     __syncthreads();
-    build_tables<N, T>(g, s_mom, s_P, s_E, s_s2);
+    build_tables<N, T, G>(g, s_mom, s_P, s_E, s_s2);
 }
 
 // a8: |ampsum|^2 summed over the event's 2^N lanes (warp shuffles, one shared-memory pass for
 // N > 5), times the constant factors, one store per event.
-template <int N, typename T>
+template <int N, typename T, typename G = Geometry<N>>
 __device__ __forceinline__ void finish_event(T ar, T ai, const double* s_mom, const double* s_s2, double* s_red,
                                              double g, double* __restrict__ out, int64_t ev0, int64_t n_events)
 {
-    using G = Geometry<N>;
     constexpr int MOM = 4 * (N + 2);
     const int tid = threadIdx.x;
     const int ev_local = tid / G::L;

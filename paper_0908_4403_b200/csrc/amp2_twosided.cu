@@ -190,7 +190,8 @@ struct TwoSidedSmem {
 #define HEGET_TS_MINB64 1
 #endif
 template <int N, typename T>
-__global__ void __launch_bounds__(Geometry<N>::THREADS, (sizeof(T) == 4) ? HEGET_TS_MINB32 : HEGET_TS_MINB64)
+__global__ void __launch_bounds__(Geometry<N>::THREADS,
+                                  ((sizeof(T) == 4) ? HEGET_TS_MINB32 : HEGET_TS_MINB64) * 256 / Geometry<N>::THREADS)
 amp2_twosided_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_t n_events, double g)
 {
     using G = Geometry<N>;
