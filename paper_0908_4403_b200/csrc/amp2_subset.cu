@@ -22,6 +22,13 @@
 #include "amp2_common.cuh"
 #include "subset_index.cuh"
 
+// CTA size ("CTA size"): measured on B200, 256 -> 128 threads: 4 gamma 0.449 -> 0.436 ms fp32, 5 gamma 1.50 -> 1.43 ms
+#ifndef HEGET_SUBSET_CTA_THREADS
+#define HEGET_SUBSET_CTA_THREADS 128
+#endif
+template <int N>
+using KGeometry = Geometry<N, HEGET_SUBSET_CTA_THREADS>;
+
 namespace {
 
 template <int N>
@@ -132,7 +139,7 @@ struct Levels {
 
 template <int N, typename T>
 struct SubsetSmem {
-    using G = Geometry<N>;
+    using G = KGeometry<N>;
     static constexpr int MOM = 4 * (N + 2);
     static constexpr int LVL = max_level_items<N>();
     // byte offsets, every array 16-byte aligned (32 for the double spinors)
@@ -149,10 +156,10 @@ struct SubsetSmem {
 };
 
 template <int N, typename T>
-__global__ void __launch_bounds__(Geometry<N>::THREADS)
+__global__ void __launch_bounds__(KGeometry<N>::THREADS)
 amp2_subset_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_t n_events, double g)
 {
-    using G = Geometry<N>;
+    using G = KGeometry<N>;
     using SM = SubsetSmem<N, T>;
     extern __shared__ __align__(32) unsigned char smem[];
     Spinor<T>* s_psi0 = reinterpret_cast<Spinor<T>*>(smem + SM::off_psi0);
@@ -169,7 +176,7 @@ amp2_subset_kernel(const double* __restrict__ momenta, double* __restrict__ out,
     const unsigned hel = threadIdx.x % G::L;
 
     load_subset_index<N, G::THREADS>(s_rank, s_list);
-    build_event_tables<N, T>(momenta, (int64_t)blockIdx.x * G::EPB, n_events, g, s_mom, s_P, s_E, s_s2);  // ends with a barrier
+    build_event_tables<N, T, G>(momenta, (int64_t)blockIdx.x * G::EPB, n_events, g, s_mom, s_P, s_E, s_s2);  // ends with a barrier
 
     const PEntry<T>* P = s_P + ev_local * G::L;
     const EEntry<T>* E = s_E + ev_local * 2 * N;
@@ -189,13 +196,13 @@ amp2_subset_kernel(const double* __restrict__ momenta, double* __restrict__ out,
         ar += fma(e.ar, f.r0, fma(-e.ai, f.i0, f.r1));
         ai += fma(e.ar, f.i0, fma(e.ai, f.r0, f.i1));
     }
-    finish_event<N, T>(ar, ai, s_mom, s_s2, s_red, g, out, (int64_t)blockIdx.x * G::EPB, n_events);
+    finish_event<N, T, G>(ar, ai, s_mom, s_s2, s_red, g, out, (int64_t)blockIdx.x * G::EPB, n_events);
 }
 
 template <int N, typename T>
 cudaError_t launch_one(const double* momenta, double* out, int64_t n_events, double g, cudaStream_t stream)
 {
-    using G = Geometry<N>;
+    using G = KGeometry<N>;
     constexpr size_t bytes = SubsetSmem<N, T>::bytes;
     if (bytes > 48 * 1024) {  // opt in to large dynamic shared memory (per device, cheap to repeat)
         cudaError_t err = cudaFuncSetAttribute(amp2_subset_kernel<N, T>, cudaFuncAttributeMaxDynamicSharedMemorySize,

@@ -19,6 +19,13 @@
 #include "amp2_tree.cuh"
 #include "subset_index.cuh"
 
+// CTA size ("CTA size"): measured on B200, 256 -> 64 threads: 4 gamma fp64 1.04 -> 0.91 ms, 6 gamma fp64 14.2 -> 12.2 ms
+#ifndef HEGET_TS_CTA_THREADS
+#define HEGET_TS_CTA_THREADS 64
+#endif
+template <int N>
+using KGeometry = Geometry<N, HEGET_TS_CTA_THREADS>;
+
 namespace {
 
 #ifndef HEGET_KSUFFIX
@@ -164,7 +171,7 @@ struct Walk2 {
 
 template <int N, typename T>
 struct TwoSidedSmem {
-    using G = Geometry<N>;
+    using G = KGeometry<N>;
     static constexpr int KS = kSuffix<N>;
     static constexpr int MOM = 4 * (N + 2);
     static constexpr int L2 = binom(N, 2) << 2;                 // entries of level 2
@@ -190,11 +197,11 @@ struct TwoSidedSmem {
 #define HEGET_TS_MINB64 1
 #endif
 template <int N, typename T>
-__global__ void __launch_bounds__(Geometry<N>::THREADS,
-                                  ((sizeof(T) == 4) ? HEGET_TS_MINB32 : HEGET_TS_MINB64) * 256 / Geometry<N>::THREADS)
+__global__ void __launch_bounds__(KGeometry<N>::THREADS,
+                                  ((sizeof(T) == 4) ? HEGET_TS_MINB32 : HEGET_TS_MINB64) * 256 / KGeometry<N>::THREADS)
 amp2_twosided_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_t n_events, double g)
 {
-    using G = Geometry<N>;
+    using G = KGeometry<N>;
     using SM = TwoSidedSmem<N, T>;
     constexpr int KS = SM::KS;
     constexpr int RB = (N < KS + 2) ? N : KS + 2;  // remaining photons where unrolling starts
@@ -215,7 +222,7 @@ amp2_twosided_kernel(const double* __restrict__ momenta, double* __restrict__ ou
     const int64_t ev0 = (int64_t)blockIdx.x * G::EPB;
 
     load_subset_index<N, G::THREADS>(s_rank, s_list);
-    build_event_tables<N, T>(momenta, ev0, n_events, g, s_mom, s_P, s_E, s_s2);  // ends with a barrier
+    build_event_tables<N, T, G>(momenta, ev0, n_events, g, s_mom, s_P, s_E, s_s2);  // ends with a barrier
 
     const PEntry<T>* P = s_P + ev_local * G::L;
     const EEntry<T>* E = s_E + ev_local * 2 * N;
@@ -237,13 +244,13 @@ amp2_twosided_kernel(const double* __restrict__ momenta, double* __restrict__ ou
     T ar = 0, ai = 0;
     const Spinor<T> f0 = {(T)1, (T)0, (T)0, (T)0};
     Walk2<N, 0, RB, KS, T>::run(P, E, hel, 0u, f0, Ltab, s_rank, ar, ai);
-    finish_event<N, T>(ar, ai, s_mom, s_s2, s_red, g, out, ev0, n_events);
+    finish_event<N, T, G>(ar, ai, s_mom, s_s2, s_red, g, out, ev0, n_events);
 }
 
 template <int N, typename T>
 cudaError_t launch_one(const double* momenta, double* out, int64_t n_events, double g, cudaStream_t stream)
 {
-    using G = Geometry<N>;
+    using G = KGeometry<N>;
     constexpr size_t bytes = TwoSidedSmem<N, T>::bytes;
     if (bytes > 48 * 1024) {
         cudaError_t err = cudaFuncSetAttribute(amp2_twosided_kernel<N, T>, cudaFuncAttributeMaxDynamicSharedMemorySize,

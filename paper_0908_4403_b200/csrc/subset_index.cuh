@@ -37,10 +37,13 @@ constexpr SubsetIndex make_subset_index()
 static __constant__ SubsetIndex c_index = make_subset_index();
 
 
-// copy the index tables into shared memory: s_rank[256], s_list[(N + 1) * 72]
+// copy the part of the index tables that N photons use into shared memory:
+// s_rank[0 .. 2^N), s_list[m * 72 + r] for m <= N, r < C(N, m)   (row stride 72 as in c_index)
 template <int N, int THREADS>
 __device__ __forceinline__ void load_subset_index(unsigned char* s_rank, unsigned char* s_list)
 {
-    for (int i = threadIdx.x; i < 256; i += THREADS) s_rank[i] = c_index.rank[i];
-    for (int i = threadIdx.x; i < (N + 1) * 72; i += THREADS) s_list[i] = c_index.list[i / 72][i % 72];
+    constexpr int COLS = binom(N, N / 2);  // widest row
+    for (int i = threadIdx.x; i < (1 << N); i += THREADS) s_rank[i] = c_index.rank[i];
+    for (int i = threadIdx.x; i < (N + 1) * COLS; i += THREADS)
+        s_list[(i / COLS) * 72 + i % COLS] = c_index.list[i / COLS][i % COLS];
 }
