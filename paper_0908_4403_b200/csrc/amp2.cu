@@ -63,11 +63,14 @@ constexpr int kBottom = (N < HEGET_KB) ? N : HEGET_KB;  // unrolled bottom level
 // 0.862 -> 0.755 ms, 5 gamma 6.48 -> 6.39 ms; fp32 3 gamma and every fp64 kernel are 1-6 % SLOWER
 // that way (two 128-register CTAs per SM overlap their phases better when CTAs turn over), so
 // those keep one batch per CTA.
+#ifndef HEGET_PERSIST32
+#define HEGET_PERSIST32 1
+#endif
 #ifndef HEGET_PERSIST64_N4
 #define HEGET_PERSIST64_N4 0
 #endif
 template <int N, typename T>
-constexpr bool kPersistent = ((sizeof(T) == 4) && (N == 4 || N == 5)) || (HEGET_PERSIST64_N4 != 0 && sizeof(T) == 8 && N == 4);
+constexpr bool kPersistent = (HEGET_PERSIST32 != 0 && (sizeof(T) == 4) && (N == 4 || N == 5)) || (HEGET_PERSIST64_N4 != 0 && sizeof(T) == 8 && N == 4);
 
 template <int N, typename T>
 __global__ void __launch_bounds__(TreeGeometry<N>::THREADS,
