@@ -19,6 +19,9 @@
 #ifndef HEGET_MINB64
 #define HEGET_MINB64 2
 #endif
+#ifndef HEGET_MINW64
+#define HEGET_MINW64 (HEGET_MINB64 * 8)   // fp64: minimum resident warps per SM the register cap is set for
+#endif
 
 // CTA size of the tree kernels.  Small CTAs (64 threads: 4 events at n = 4) put more CTAs, each in
 // its own phase (load / tables / tree), on an SM at the same number of warps, which overlaps the
@@ -74,7 +77,7 @@ constexpr bool kPersistent = (HEGET_PERSIST32 != 0 && (sizeof(T) == 4) && (N == 
 
 template <int N, typename T>
 __global__ void __launch_bounds__(TreeGeometry<N>::THREADS,
-                                  ((sizeof(T) == 4) ? HEGET_MINB32 : HEGET_MINB64) * 256 / TreeGeometry<N>::THREADS)
+                                  ((sizeof(T) == 4) ? HEGET_MINB32 * 256 : HEGET_MINW64 * 32) / TreeGeometry<N>::THREADS)
 amp2_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_t n_events, double g,
             int64_t n_batches)
 {
