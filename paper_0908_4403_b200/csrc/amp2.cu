@@ -40,11 +40,14 @@ namespace {
 #define HEGET_SHARE32_MAXN 0   // fp32: lane sharing of the last level for N up to this; 0 = off (measured: no gain,
                                // 3 gamma -6 %, 4 gamma +4 %, 5-7 gamma +-1 %: the shuffles cost the issue slots they save)
 #endif
+#ifndef HEGET_SHARE64_MAXN
+#define HEGET_SHARE64_MAXN 7
+#endif
 #ifndef HEGET_SHARE64
 #define HEGET_SHARE64 1   // fp64: share the last fvixx0 of a branch between the two helicity lanes that need it
 #endif
 template <int N, typename T>
-constexpr int kShare = (sizeof(T) == 8) ? ((N <= 7) ? HEGET_SHARE64 : 0) : ((N <= HEGET_SHARE32_MAXN) ? 1 : 0);  // N = 8: too few in-warp pairs, 2 % slower
+constexpr int kShare = (sizeof(T) == 8) ? ((N <= HEGET_SHARE64_MAXN) ? HEGET_SHARE64 : 0) : ((N <= HEGET_SHARE32_MAXN) ? 1 : 0);  // N = 8: too few in-warp pairs, 2 % slower
 
 // Small N: the spinors of the first two tree levels depend on two photons' helicities only, so
 // the 2^N lanes of an event would each recompute the same N(N-1)*4 values (N = 4: 30 % of a
