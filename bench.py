@@ -38,22 +38,17 @@ def model_flops_per_event(n):
 
 def executed_flops_per_event(n, precision="fp32"):
     """What amp2_kernel executes: 2^n lanes (sigma_1 = +1 only, doubled by
-    parity), per lane one fvixx0 node = 16 FMA + 4 MUL = 36 flop per ordered prefix and one iovxxx
-    leaf = 4 FMA + 2 ADD = 10 flop per permutation.  The fp64 kernels share spinors between
-    helicity lanes: for n <= 7 the two lanes that differ in the last photon's helicity compute one
-    of the two last-level nodes each and exchange them by shuffle whenever both remaining photons
-    have index < 5 (a fraction C(min(n,5),2)/C(n,2) of the n!/2 last-but-one nodes saves one node);
-    the 4-photon kernel also computes the first two tree levels once per event (48 two-node
-    entries) instead of once per lane (16 nodes).  Tables excluded.  Cross-checked against ncu's
-    sass_thread_inst_executed_op_{f,d}{fma,mul,add} counters in profiles/."""
-    internal = sum(math.factorial(n) // math.factorial(n - l) for l in range(1, n))
-    flops = 2 ** n * (36 * internal + 10 * math.factorial(n))
-    if precision == "fp64" and 2 <= n <= 7:
-        m = min(n, 5)
-        share = (m * (m - 1) // 2) / (n * (n - 1) // 2)
-        flops -= 2 ** n * (math.factorial(n) // 2) * share * 36
-        if n == 4:
-            flops -= 2 ** n * 16 * 36 - 48 * 2 * 36
+    parity); per lane one fvixx0 node = 16 FMA + 4 MUL = 36 flop for every ordered prefix of up to
+    n-2 photons, and for each of the n!/2 prefixes of n-2 photons the two remaining orderings as
+    vertex + closing-table dot, 2 x (16 + 16) = 64 flop (the last fvixx0 + iovxxx of a branch
+    associated as <vbar|E'_b P . (E'_a psi)).  The fp64 4-photon kernel also computes the first two
+    tree levels once per event (48 two-node entries) instead of once per lane (16 nodes).  Tables
+    excluded.  Cross-checked against ncu's sass_thread_inst_executed_op_{f,d}{fma,mul,add} counters
+    in profiles/."""
+    upper = sum(math.factorial(n) // math.factorial(n - l) for l in range(1, n - 1))
+    flops = 2 ** n * (36 * upper + 64 * (math.factorial(n) // 2))
+    if precision == "fp64" and n == 4:
+        flops -= 2 ** n * 16 * 36 - 48 * 2 * 36
     return flops
 
 
@@ -363,12 +358,13 @@ def main():
                 "model_c_tflops": model_c / 1e12, "model_c_frac": model_c / peak_measured,
                 "frac_note": "frac counts EXECUTED flops (what ncu counts); model_c_frac counts SURVEY 8(d)'s fixed "
                              "algorithmic figure (model C) over the same time.  Work removed by the parity relation and "
-                             "by sharing spinors between helicity lanes lowers frac while events/s and model_c_frac "
-                             "rise (4 gamma fp64: v3 1.48 ms, frac 0.56 -> v4 1.19 ms, frac 0.37)",
-                "flops_model": "executed: 2^n lanes x (36 flop per tree node + 10 per leaf), minus the nodes the fp64 "
-                               "kernels share between helicity lanes (see executed_flops_per_event); model C (SURVEY "
-                               "8(d)): 2*2^n x (44 per node + 24 per leaf), 2.5-5x the executed count because the kernel "
-                               "evaluates sigma_1=+1 only (parity) with normalised polarisation blocks"}
+                             "by re-associating or sharing factors lowers frac while events/s and model_c_frac rise "
+                             "(4 gamma fp64: v3 1.48 ms, frac 0.56 -> v7 1.02 ms, frac 0.38)",
+                "flops_model": "executed: 2^n lanes x (36 flop per tree node down to depth n-2 + 64 per pair of last "
+                               "orderings), see executed_flops_per_event; model C (SURVEY 8(d)): 2*2^n x (44 per node "
+                               "+ 24 per leaf), 3-5x the executed count because the kernel evaluates sigma_1=+1 only "
+                               "(parity), uses normalised polarisation blocks and contracts the last propagator into "
+                               "the closing vertex"}
 
     result = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
               "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,

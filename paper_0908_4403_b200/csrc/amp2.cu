@@ -40,11 +40,16 @@ namespace {
 #define HEGET_SHARE32_MAXN 0   // fp32: lane sharing of the last level for N up to this; 0 = off (measured: no gain,
                                // 3 gamma -6 %, 4 gamma +4 %, 5-7 gamma +-1 %: the shuffles cost the issue slots they save)
 #endif
+#ifndef HEGET_CLOSE
+#define HEGET_CLOSE 1   // last fvixx0 + iovxxx of a branch as vertex + closing-table dot (amp2_tree.cuh)
+#endif
 #ifndef HEGET_SHARE64_MAXN
 #define HEGET_SHARE64_MAXN 7
 #endif
 #ifndef HEGET_SHARE64
-#define HEGET_SHARE64 1   // fp64: share the last fvixx0 of a branch between the two helicity lanes that need it
+#define HEGET_SHARE64 0   // fp64: share the last vertex of a branch between the two helicity lanes that need it
+                          // (v4: -8 % at 4 gamma; since the closing table (HEGET_CLOSE) halves that level's work
+                          // it costs 1-3 % at 5-7 gamma and gains < 1 % at 4 gamma: off)
 #endif
 template <int N, typename T>
 constexpr int kShare = (sizeof(T) == 8) ? ((N <= HEGET_SHARE64_MAXN) ? HEGET_SHARE64 : 0) : ((N <= HEGET_SHARE32_MAXN) ? 1 : 0);  // N = 8: too few in-warp pairs, 2 % slower
@@ -92,6 +97,7 @@ amp2_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_
     __shared__ EEntry<T> s_E[G::EPB * 2 * N];
     __shared__ double s_red[G::THREADS / 32];
     __shared__ double s_s2[G::EPB * N];  // s_i^2 = (pT/w)^2 taken out of photon i's E entries
+    __shared__ Spinor<T> s_U[G::EPB * 2 * N];  // closing table (amp2_tree.cuh, close_weyl)
     constexpr int TOP = kTopShare<N, T> ? N * (N - 1) * 4 : 1;  // psi_2 entries per event
     __shared__ Spinor<T> s_top[kTopShare<N, T> ? G::EPB * TOP : 1];
 
@@ -108,6 +114,7 @@ amp2_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_
             if (batch + gridDim.x < n_batches) Tile::load(momenta, (batch + gridDim.x) * G::EPB, n_events, pf);
         }
         build_tables<N, T, G>(g, s_mom, s_P, s_E, s_s2);                        // a4, a5 (ends with a barrier)
+        if constexpr (HEGET_CLOSE != 0) build_closing_table<N, T, G>(s_P, s_E, s_U);
 
         // a2, a6, a7: psi_0 = u(p1,+)/sqrt(2E1) = (1,0); walk the permutation tree
         T ar = 0, ai = 0;
@@ -129,10 +136,11 @@ amp2_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_
                 for (int jj = 0; jj < N - 1; ++jj) {
                     const int j = jj + (jj >= i ? 1 : 0);
                     const Spinor<T> f2 = top[(i * (N - 1) + jj) * 4 + 2 * ((hel >> i) & 1u) + ((hel >> j) & 1u)];
-                    Walk<N, 2, N - 2, T, kShare<N, T>>::run(P, E, hel, (1u << i) | (1u << j), f2, ar, ai);
+                    Walk<N, 2, N - 2, T, kShare<N, T>, HEGET_CLOSE>::run(P, E, hel, (1u << i) | (1u << j), f2, ar, ai,
+                                                                        s_U + ev_local * 2 * N);
                 }
         } else {
-            Walk<N, 0, kBottom<N>, T, kShare<N, T>>::run(P, E, hel, 0u, f0, ar, ai);
+            Walk<N, 0, kBottom<N>, T, kShare<N, T>, HEGET_CLOSE>::run(P, E, hel, 0u, f0, ar, ai, s_U + ev_local * 2 * N);
         }
 
         // a8: |ampsum|^2 summed over the event's 2^N lanes, constant factors, store

@@ -44,6 +44,31 @@ __device__ __forceinline__ void iovxxx_weyl(const EEntry<T>& E, const Spinor<T>&
     ai += fma(E.ar, f.i0, fma(E.ai, f.r0, f.i1));
 }
 
+// The FFV vertex alone, w = E' psi (8 FMA-pipe instructions), and the closing of a branch whose
+// last propagator has been contracted into the closing vertex:
+//   <vbar| E'_b P_{all \ b} (E'_a psi) = U_b . (E'_a psi),   U_b = <vbar| E'_b P_{all \ b}
+// (the last propagator of EVERY ordering that ends with photon b belongs to the set "all but b",
+// so U_b is one row vector per photon and helicity: build_closing_table, amp2_common.cuh).
+// The product of the last three factors of a diagram is merely associated differently:
+// 8 + 8 instructions for the last fvixx0 + iovxxx of a branch instead of 20 + 6.
+template <typename T>
+__device__ __forceinline__ Spinor<T> vertex_weyl(const EEntry<T>& E, const Spinor<T>& f)
+{
+    Spinor<T> w;
+    w.r0 = fma(-E.br, f.r1, fma(E.bi, f.i1, -f.r0));
+    w.i0 = fma(-E.br, f.i1, fma(-E.bi, f.r1, -f.i0));
+    w.r1 = fma(E.ar, f.r0, fma(-E.ai, f.i0, f.r1));
+    w.i1 = fma(E.ar, f.i0, fma(E.ai, f.r0, f.i1));
+    return w;
+}
+
+template <typename T>
+__device__ __forceinline__ void close_weyl(const Spinor<T>& U, const Spinor<T>& w, T& ar, T& ai)
+{
+    ar += fma(U.r0, w.r0, fma(-U.i0, w.i0, fma(U.r1, w.r1, -(U.i1 * w.i1))));
+    ai += fma(U.r0, w.i0, fma(U.i0, w.r0, fma(U.r1, w.i1, U.i1 * w.r1)));
+}
+
 // Bottom K levels of the permutation tree, fully unrolled.  The K photons still to attach are
 // held as compile-time-indexed register arrays (bit[] = their subset-index bits, e[] = this
 // lane's E' entries), so choosing a child is register renaming, not bit arithmetic: the code
@@ -70,12 +95,37 @@ __device__ __forceinline__ EEntry<T> eselect(bool c, const EEntry<T>* a, const E
 // Needs both photons' lane bits inside the warp (photon index < 5); otherwise, and always for
 // SHARE = 0 (fp32, where the shuffles would cost what they save; amp2_sampled.cu, whose lanes are
 // not helicity configurations), both nodes are computed.  hb[] = this lane's helicity bits.
-template <int K, typename T, typename EA, int SHARE = 0>
+// CLOSE = 1: the last fvixx0 + iovxxx of every branch are evaluated as vertex + close_weyl with
+// the closing table (u[] = this lane's U entries of the remaining photons).
+template <int K, typename T, typename EA, int SHARE = 0, int CLOSE = 0>
 struct Bottom {
     static __device__ __forceinline__ void run(const PEntry<T>* __restrict__ PS, const int (&bit)[K],
-                                               const EA (&e)[K], const unsigned (&hb)[K], const Spinor<T>& f,
-                                               T& ar, T& ai)
+                                               const EA (&e)[K], const unsigned (&hb)[K],
+                                               const Spinor<T>* const (&u)[K], const Spinor<T>& f, T& ar, T& ai)
     {
+        if constexpr (K == 2 && CLOSE == 1) {
+            if constexpr (SHARE == 1) {
+                if ((bit[0] | bit[1]) < 32) {  // uniform over the CTA
+                    // w_a = E'_a psi does not depend on the helicity of b (and vice versa): each lane
+                    // evaluates one of the two vertices and fetches the other one by shuffle
+                    const bool odd = (hb[0] ^ hb[1]) != 0u;
+                    const EEntry<T> em = eselect<T>(odd, e[1], e[0]);
+                    const int bm = odd ? bit[1] : bit[0];
+                    const Spinor<T> wm = vertex_weyl(em, f);
+                    Spinor<T> wo;
+                    wo.r0 = __shfl_xor_sync(0xffffffffu, wm.r0, bm);
+                    wo.i0 = __shfl_xor_sync(0xffffffffu, wm.i0, bm);
+                    wo.r1 = __shfl_xor_sync(0xffffffffu, wm.r1, bm);
+                    wo.i1 = __shfl_xor_sync(0xffffffffu, wm.i1, bm);
+                    close_weyl(*(odd ? u[0] : u[1]), wm, ar, ai);  // my vertex closes with the other photon
+                    close_weyl(*(odd ? u[1] : u[0]), wo, ar, ai);  // the received one closes with mine
+                    return;
+                }
+            }
+            close_weyl(*u[1], vertex_weyl(eload<T>(e[0]), f), ar, ai);
+            close_weyl(*u[0], vertex_weyl(eload<T>(e[1]), f), ar, ai);
+            return;
+        }
         if constexpr (K == 2 && SHARE == 1) {
             if ((bit[0] | bit[1]) < 32) {  // uniform over the CTA
                 const bool odd = (hb[0] ^ hb[1]) != 0u;
@@ -100,24 +150,26 @@ struct Bottom {
             int sub_bit[K - 1];
             EA sub_e[K - 1];
             unsigned sub_hb[K - 1];
+            const Spinor<T>* sub_u[K - 1];
 #pragma unroll
             for (int m = 0; m < K - 1; ++m) {
                 sub_bit[m] = bit[m + (m >= i ? 1 : 0)];
                 sub_e[m] = e[m + (m >= i ? 1 : 0)];
                 sub_hb[m] = hb[m + (m >= i ? 1 : 0)];
+                sub_u[m] = u[m + (m >= i ? 1 : 0)];
             }
             const PEntry<T>* Pn = PS + bit[i];
             const Spinor<T> fn = fvixx0_weyl(*Pn, eload<T>(e[i]), f);
-            Bottom<K - 1, T, EA, SHARE>::run(Pn, sub_bit, sub_e, sub_hb, fn, ar, ai);
+            Bottom<K - 1, T, EA, SHARE, CLOSE>::run(Pn, sub_bit, sub_e, sub_hb, sub_u, fn, ar, ai);
         }
     }
 };
 
-template <typename T, typename EA, int SHARE>
-struct Bottom<1, T, EA, SHARE> {
+template <typename T, typename EA, int SHARE, int CLOSE>
+struct Bottom<1, T, EA, SHARE, CLOSE> {
     static __device__ __forceinline__ void run(const PEntry<T>* __restrict__, const int (&)[1],
-                                               const EA (&e)[1], const unsigned (&)[1], const Spinor<T>& f,
-                                               T& ar, T& ai)
+                                               const EA (&e)[1], const unsigned (&)[1],
+                                               const Spinor<T>* const (&)[1], const Spinor<T>& f, T& ar, T& ai)
     {
         iovxxx_weyl(eload<T>(e[0]), f, ar, ai);
     }
@@ -125,11 +177,13 @@ struct Bottom<1, T, EA, SHARE> {
 
 // Depth-first walk of the upper levels.  `used` = set of photons already attached (uniform
 // over the CTA); when KB photons remain the unrolled Bottom<KB> takes over.
-template <int N, int DEPTH, int KB, typename T, int SHARE = 0>
+template <int N, int DEPTH, int KB, typename T, int SHARE = 0, int CLOSE = 0>
 struct Walk {
     static __device__ __forceinline__ void run(const PEntry<T>* __restrict__ P, const EEntry<T>* __restrict__ E,
-                                               unsigned hel, unsigned used, const Spinor<T>& f, T& ar, T& ai)
+                                               unsigned hel, unsigned used, const Spinor<T>& f, T& ar, T& ai,
+                                               const Spinor<T>* __restrict__ U = nullptr)
     {
+        static_assert(CLOSE == 0 || KB >= 2, "the closing table replaces the last TWO levels");
         unsigned avail = ((1u << N) - 1u) & ~used;
         if constexpr (N - DEPTH == KB) {
             int bit[KB];
@@ -139,25 +193,27 @@ struct Walk {
             constexpr bool BY_PTR = (HEGET_E_BY_PTR != 0) || (SHARE == 1 && HEGET_SHARE_BY_PTR != 0);
             using EA = std::conditional_t<BY_PTR, const EEntry<T>*, EEntry<T>>;
             EA e[KB];
+            const Spinor<T>* u[KB];
 #pragma unroll
             for (int m = 0; m < KB; ++m) {
                 const int i = __ffs(avail) - 1;
                 avail &= avail - 1u;
                 bit[m] = 1 << i;
                 hb[m] = (hel >> i) & 1u;
+                u[m] = U + 2 * i + hb[m];
                 if constexpr (BY_PTR)
                     e[m] = &E[2 * i + hb[m]];
                 else
                     e[m] = E[2 * i + hb[m]];
             }
-            Bottom<KB, T, EA, SHARE>::run(P + used, bit, e, hb, f, ar, ai);
+            Bottom<KB, T, EA, SHARE, CLOSE>::run(P + used, bit, e, hb, u, f, ar, ai);
         } else {
             while (avail) {
                 const int i = __ffs(avail) - 1;
                 avail &= avail - 1u;
                 const unsigned S = used | (1u << i);
                 const Spinor<T> fn = fvixx0_weyl(P[S], E[2 * i + ((hel >> i) & 1u)], f);
-                Walk<N, DEPTH + 1, KB, T, SHARE>::run(P, E, hel, S, fn, ar, ai);
+                Walk<N, DEPTH + 1, KB, T, SHARE, CLOSE>::run(P, E, hel, S, fn, ar, ai, U);
             }
         }
     }

@@ -38,10 +38,14 @@ def test_flop_models_match_the_node_counts_of_the_survey():
     internal = {2: 2, 3: 9, 4: 40, 5: 205, 6: 1236, 7: 8659, 8: 69280}
     for n, nodes in internal.items():
         assert bench.model_flops_per_event(n) == 2 * 2 ** n * (44 * nodes + 24 * math.factorial(n))
-        assert bench.executed_flops_per_event(n, "fp32") == 2 ** n * (36 * nodes + 10 * math.factorial(n))
+        upper = nodes - math.factorial(n)            # prefixes of up to n-2 photons
+        assert bench.executed_flops_per_event(n, "fp32") == 2 ** n * (36 * upper + 32 * math.factorial(n))
         assert bench.executed_flops_per_event(n, "fp64") <= bench.executed_flops_per_event(n, "fp32")
         for algo in ("subset", "two-sided"):
-            assert 0 < bench.executed_flops_per_event_algo(n, algo) <= bench.executed_flops_per_event(n, "fp32") * 1.1
+            # never more work than the one-sided tree once there is a tree to speak of
+            assert 0 < bench.executed_flops_per_event_algo(n, algo)
+            if n >= 4:
+                assert bench.executed_flops_per_event_algo(n, algo) <= bench.executed_flops_per_event(n, "fp32")
     # model C as tabulated in SURVEY 8(d): 1.09e3, 7.5e4, 2.06e9 flop per event
     assert abs(bench.model_flops_per_event(2) / 1.09e3 - 1) < 0.01
     assert abs(bench.model_flops_per_event(4) / 7.5e4 - 1) < 0.01
