@@ -109,21 +109,25 @@ __device__ __forceinline__ void build_tables(double g, const double* s_mom, PEnt
 // Closing table: U[2 b + h] = <vbar| E'_b(h) P_{all \ b} = (a pp + q, a qbar + pm), one row vector per
 // photon and helicity (amp2_tree.cuh, close_weyl).  Reads s_P and s_E (barrier before), ends with
 // a barrier.
+template <typename T>
+__device__ __forceinline__ Spinor<T> closing_entry(const EEntry<T>& e, const PEntry<T>& p)
+{
+    Spinor<T> u;  // (a, 1) . [[pp, px - i py], [px + i py, pm]]
+    u.r0 = fma(e.ar, p.pp, p.px);
+    u.i0 = fma(e.ai, p.pp, p.py);
+    u.r1 = fma(e.ar, p.px, fma(e.ai, p.py, p.pm));
+    u.i1 = fma(e.ai, p.px, -(e.ar * p.py));
+    return u;
+}
+
 template <int N, typename T, typename G = Geometry<N>>
 __device__ __forceinline__ void build_closing_table(const PEntry<T>* s_P, const EEntry<T>* s_E, Spinor<T>* s_U)
 {
     const int ev_local = threadIdx.x / G::L;
     const unsigned lane = threadIdx.x % G::L;
-    for (unsigned q = lane; q < 2u * N; q += G::L) {
-        const EEntry<T> e = s_E[ev_local * 2 * N + q];
-        const PEntry<T> p = s_P[ev_local * G::L + ((G::L - 1) ^ (1u << (q >> 1)))];
-        Spinor<T> u;
-        u.r0 = fma(e.ar, p.pp, p.px);
-        u.i0 = fma(e.ai, p.pp, p.py);
-        u.r1 = fma(e.ar, p.px, fma(e.ai, p.py, p.pm));
-        u.i1 = fma(e.ai, p.px, -(e.ar * p.py));
-        s_U[ev_local * 2 * N + q] = u;
-    }
+    for (unsigned q = lane; q < 2u * N; q += G::L)
+        s_U[ev_local * 2 * N + q] = closing_entry(s_E[ev_local * 2 * N + q],
+                                                  s_P[ev_local * G::L + ((G::L - 1) ^ (1u << (q >> 1)))]);
     __syncthreads();
 }
 

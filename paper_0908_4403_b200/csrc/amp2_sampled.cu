@@ -55,6 +55,7 @@ amp2_sampled_kernel(const double* __restrict__ momenta, uint64_t seed, uint64_t 
     __shared__ PEntry<T> s_P[EPB * L];
     __shared__ EEntry<T> s_E[EPB * 2 * N];
     __shared__ double s_s2[EPB * N];
+    __shared__ Spinor<T> s_U[EPB * 2 * N];  // closing table (amp2_tree.cuh, close_weyl)
 
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const int64_t ev0 = (int64_t)blockIdx.x * EPB;
@@ -82,6 +83,8 @@ amp2_sampled_kernel(const double* __restrict__ momenta, uint64_t seed, uint64_t 
             make_subset_entry<N, T>(mom, S, g, scale, &P[S]);
     }
     __syncthreads();
+    if (lane < 2 * N) s_U[w * 2 * N + lane] = closing_entry(E[lane], P[(L - 1) ^ (1 << (lane >> 1))]);
+    __syncthreads();
 
     const int64_t e = ev0 + w;
     const uint64_t gev = first_event + (uint64_t)(e < n_events ? e : n_events - 1);
@@ -107,7 +110,7 @@ amp2_sampled_kernel(const double* __restrict__ momenta, uint64_t seed, uint64_t 
                 used |= 1u << i;
                 f = fvixx0_weyl(P[used], E[2 * i + ((hel >> i) & 1u)], f);
             }
-            Walk<N, D, KB, T>::run(P, E, hel, used, f, ar, ai);
+            Walk<N, D, KB, T, 0, (KB >= 2) ? 1 : 0>::run(P, E, hel, used, f, ar, ai, s_U + w * 2 * N);
         }
     }
     double dr = (double)ar, di = (double)ai;
@@ -185,9 +188,12 @@ amp2_sampled_thread_kernel(const double* __restrict__ momenta, uint64_t seed, ui
             else
                 make_subset_entry<N, T>(mom, S, g, scale, &P[S]);
         }
+        Spinor<T> U[2 * N];
+#pragma unroll
+        for (int q = 0; q < 2 * N; ++q) U[q] = closing_entry(E[q], P[(L - 1) ^ (1 << (q >> 1))]);
         T ar = 0, ai = 0;
         const Spinor<T> f0 = {(T)1, (T)0, (T)0, (T)0};
-        Walk<N, 0, N, T>::run(P, E, hel, 0u, f0, ar, ai);
+        Walk<N, 0, N, T, 0, 1>::run(P, E, hel, 0u, f0, ar, ai, U);
         if (sizeof(T) == 4) {
             const double inv = 1.0 / shat;
 #pragma unroll
