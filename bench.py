@@ -60,16 +60,23 @@ def executed_flops_per_event_algo(n, algo, precision="fp32"):
     """Executed flops of the separately named algorithms, tables excluded.
     subset: level m holds C(n,m) 2^m items of m vertex accumulations (8 FMA + 4 ADD = 20 flop) and
     one propagator (8 FMA + 4 MUL = 20 flop); 2^n closings of n terms (4 FMA + 2 ADD = 10 flop).
-    two-sided: per lane the tree to depth n-KS (36 flop per node) and n!/KS! closings (16 flop),
-    plus the ubar-side table, C(n,m) 2^m entries of m x 40 flop for m = 2..KS, KS = min(n,4)."""
+    two-sided: per lane the tree to depth n-KS-1 (36 flop per node) and n!/KS! closings of a vertex and a
+    dot product (32 flop), plus the ubar-side table, C(n,m) 2^m entries of m x 40 flop for m = 2..KS and
+    the folded last propagator (20 flop per entry of level KS), KS = min(n,4)."""
     if algo == "tree":
         return executed_flops_per_event(n, precision)
     if algo == "subset":
         return sum(_binom(n, m) * 2 ** m * (20 * m + 20) for m in range(1, n)) + 2 ** n * 10 * n
     ks = min(n, 4)
-    nodes = sum(math.factorial(n) // math.factorial(n - l) for l in range(1, n - ks + 1))
-    per_lane = 36 * nodes + 16 * (math.factorial(n) // math.factorial(ks))
+    closings = math.factorial(n) // math.factorial(ks)
+    if ks == n:                                   # no u-side tree: one dot product per lane
+        per_lane = 16 * closings
+    else:                                         # full nodes above the last u-side photon, vertex + dot there
+        nodes = sum(math.factorial(n) // math.factorial(n - l) for l in range(1, n - ks))
+        per_lane = 36 * nodes + 32 * closings
     table = sum(_binom(n, m) * 2 ** m * m * 40 for m in range(2, ks + 1))
+    if ks < n:
+        table += _binom(n, ks) * 2 ** ks * 20     # last propagator folded into the table
     return 2 ** n * per_lane + table
 
 

@@ -12,7 +12,8 @@
 //   * from the u end, the depth-first permutation tree of amp2.cu is walked only to depth n - KS
 //     (each ordered prefix once), and every node at that depth closes with ONE dot product
 //         ampsum += L_KS[remaining photons] . psi
-//     instead of the KS! orderings below it.
+//     instead of the KS! orderings below it (the propagator of that last u-side node is folded into
+//     the table entry, L'[T] = L[T] P_{all \\ T}, so the node itself is only its vertex).
 // Per helicity configuration: sum_{l=1}^{n-KS} n!/(n-l)! fvixx0 nodes and n!/KS! closings
 // (n = 8: 2 080 + 1 680 against 69 280 + 40 320 in the one-sided tree).  Same E' / P tables,
 // parity shortcut, lane mapping (one lane per helicity configuration) and epilogue as amp2.cu.
@@ -58,7 +59,10 @@ __device__ __forceinline__ void accumulate_row_times_E(const Spinor<T>& r, const
 
 // Level M >= 2 of the ubar-side table from level M - 1 (M = 2: from L_1[j] = (a_j, 1)).
 // Entry q = rank(T) * 2^M + h, h compact: bit j of h = helicity of the j-th lowest photon of T.
-template <int N, int M, typename T>
+// FOLD: multiply the finished row vector by the propagator of the complementary set,
+// L'[T] = L[T] P_{all \ T}; used for the last level when a u-side tree remains (KS < N), whose
+// last fvixx0 then reduces to its vertex (the same re-association as the closing table of amp2.cu).
+template <int N, int M, typename T, bool FOLD = false>
 __device__ __forceinline__ void build_suffix_level(const PEntry<T>* __restrict__ P, const EEntry<T>* __restrict__ E,
                                                    const unsigned char* __restrict__ s_rank,
                                                    const unsigned char* __restrict__ s_list,
@@ -90,6 +94,7 @@ __device__ __forceinline__ void build_suffix_level(const PEntry<T>* __restrict__
             const Spinor<T> rp = row_times_P(r, P[FULL ^ child]);
             accumulate_row_times_E(rp, E[2 * x + ((h >> j) & 1u)], acc);
         }
+        if constexpr (FOLD) acc = row_times_P(acc, P[FULL ^ Tset]);
         cur[q] = acc;
     }
 }
@@ -98,7 +103,7 @@ __device__ __forceinline__ void build_suffix_level(const PEntry<T>* __restrict__
 // closes with the tabulated ubar-side row vector.  The remaining photons are compile-time-indexed
 // register lists in ascending photon order: bit[] = subset-index bits, e[] = this lane's E'
 // entry pointers, hb[] = this lane's helicity bits.
-template <int R, int KS, typename T>
+template <int R, int KS, typename T, bool FOLD = false>
 struct Close {
     static __device__ __forceinline__ void run(const PEntry<T>* __restrict__ PS, const int (&bit)[R],
                                                const EEntry<T>* const (&e)[R], const unsigned (&hb)[R],
@@ -127,16 +132,27 @@ struct Close {
                     sub_e[m] = e[m + (m >= i ? 1 : 0)];
                     sub_hb[m] = hb[m + (m >= i ? 1 : 0)];
                 }
-                const PEntry<T>* Pn = PS + bit[i];
-                const Spinor<T> fn = fvixx0_weyl(*Pn, *e[i], f);
-                Close<R - 1, KS, T>::run(Pn, sub_bit, sub_e, sub_hb, fn, Ltab, s_rank, ar, ai);
+                if constexpr (FOLD && R == KS + 1) {
+                    // last u-side photon: its propagator is already in the table entry
+                    unsigned Tset = 0u, h = 0u;
+#pragma unroll
+                    for (int m = 0; m < R - 1; ++m) {
+                        Tset |= (unsigned)sub_bit[m];
+                        h |= sub_hb[m] << m;
+                    }
+                    close_weyl(Ltab[((unsigned)s_rank[Tset] << KS) + h], vertex_weyl(*e[i], f), ar, ai);
+                } else {
+                    const PEntry<T>* Pn = PS + bit[i];
+                    const Spinor<T> fn = fvixx0_weyl(*Pn, *e[i], f);
+                    Close<R - 1, KS, T, FOLD>::run(Pn, sub_bit, sub_e, sub_hb, fn, Ltab, s_rank, ar, ai);
+                }
             }
         }
     }
 };
 
 // Looped upper levels; when RB photons remain the unrolled Close<RB, KS> takes over.
-template <int N, int DEPTH, int RB, int KS, typename T>
+template <int N, int DEPTH, int RB, int KS, typename T, bool FOLD = false>
 struct Walk2 {
     static __device__ __forceinline__ void run(const PEntry<T>* __restrict__ P, const EEntry<T>* __restrict__ E,
                                                unsigned hel, unsigned used, const Spinor<T>& f,
@@ -156,14 +172,14 @@ struct Walk2 {
                 hb[m] = (hel >> i) & 1u;
                 e[m] = &E[2 * i + hb[m]];
             }
-            Close<RB, KS, T>::run(P + used, bit, e, hb, f, Ltab, s_rank, ar, ai);
+            Close<RB, KS, T, FOLD>::run(P + used, bit, e, hb, f, Ltab, s_rank, ar, ai);
         } else {
             while (avail) {
                 const int i = __ffs(avail) - 1;
                 avail &= avail - 1u;
                 const unsigned S = used | (1u << i);
                 const Spinor<T> fn = fvixx0_weyl(P[S], E[2 * i + ((hel >> i) & 1u)], f);
-                Walk2<N, DEPTH + 1, RB, KS, T>::run(P, E, hel, S, fn, Ltab, s_rank, ar, ai);
+                Walk2<N, DEPTH + 1, RB, KS, T, FOLD>::run(P, E, hel, S, fn, Ltab, s_rank, ar, ai);
             }
         }
     }
@@ -229,21 +245,22 @@ amp2_twosided_kernel(const double* __restrict__ momenta, double* __restrict__ ou
     Spinor<T>* l2 = s_l2 + ev_local * SM::L2;
     Spinor<T>* l3 = s_l3 + ev_local * SM::L3;
     Spinor<T>* l4 = s_l4 + ev_local * SM::L4;
-    build_suffix_level<N, 2, T>(P, E, s_rank, s_list, nullptr, l2, hel);
+    constexpr bool FOLD = (KS < N);  // a u-side tree remains: fold its last propagator into the table
+    build_suffix_level<N, 2, T, FOLD && KS == 2>(P, E, s_rank, s_list, nullptr, l2, hel);
     __syncthreads();
     if constexpr (KS >= 3) {
-        build_suffix_level<N, 3, T>(P, E, s_rank, s_list, l2, l3, hel);
+        build_suffix_level<N, 3, T, FOLD && KS == 3>(P, E, s_rank, s_list, l2, l3, hel);
         __syncthreads();
     }
     if constexpr (KS >= 4) {
-        build_suffix_level<N, 4, T>(P, E, s_rank, s_list, l3, l4, hel);
+        build_suffix_level<N, 4, T, FOLD && KS == 4>(P, E, s_rank, s_list, l3, l4, hel);
         __syncthreads();
     }
     const Spinor<T>* Ltab = (KS >= 4) ? l4 : (KS >= 3) ? l3 : l2;
 
     T ar = 0, ai = 0;
     const Spinor<T> f0 = {(T)1, (T)0, (T)0, (T)0};
-    Walk2<N, 0, RB, KS, T>::run(P, E, hel, 0u, f0, Ltab, s_rank, ar, ai);
+    Walk2<N, 0, RB, KS, T, FOLD>::run(P, E, hel, 0u, f0, Ltab, s_rank, ar, ai);
     finish_event<N, T, G>(ar, ai, s_mom, s_s2, s_red, g, out, ev0, n_events);
 }
 
