@@ -38,10 +38,16 @@ enum { HEGET_FP32 = 0, HEGET_FP64 = 1 };
 
 enum {
     HEGET_OK = 0,
-    HEGET_EINVAL = -1, /* n outside [2,8], N < 0, null pointer, bad precision/mode */
+    HEGET_EINVAL = -1, /* n outside [2,8], N < 0 or > HEGET_MAX_EVENTS, null pointer, bad precision/mode */
     HEGET_ECUDA = -2,  /* a CUDA runtime call or launch failed */
     HEGET_ENOMEM = -3  /* host or device allocation failed */
 };
+
+/* Largest N (events, or items of the heget_helas_* calls) one call accepts: the kernels that give
+ * an event a CTA of its own (n >= 6) are launched on a grid of N blocks and CUDA's grid limit is
+ * 2^31 - 1.  A larger batch is cut by the caller (per-event results do not depend on the cut);
+ * at 32 (n + 2) bytes of momenta per event such a batch does not fit one B200 anyway. */
+#define HEGET_MAX_EVENTS 2147483647LL
 
 /* Event-generation modes of heget_gen_events ("input recipe"). */
 enum {

@@ -103,7 +103,7 @@ const char* heget_strerror(int code)
 {
     switch (code) {
         case HEGET_OK: return "success";
-        case HEGET_EINVAL: return "invalid argument (n outside [2,8], N < 0, null pointer, bad precision or mode)";
+        case HEGET_EINVAL: return "invalid argument (n outside [2,8], N < 0 || N > HEGET_MAX_EVENTS, null pointer, bad precision or mode)";
         case HEGET_ECUDA: return "CUDA runtime error (see heget_last_cuda_error)";
         case HEGET_ENOMEM: return "allocation failed";
         default: return "unknown heget error code";
@@ -117,7 +117,7 @@ int64_t heget_launch_count(const heget_ctx* ctx) { return ctx ? ctx->launches : 
 int heget_gen_events(heget_ctx* ctx, uint64_t seed, int n, const heget_gen_cfg* cfg, uint64_t first_event,
                      int64_t N, double* momenta, double* weight, void* stream)
 {
-    if (!ctx || !cfg || n < 2 || n > 8 || N < 0 || (N > 0 && !momenta)) return HEGET_EINVAL;
+    if (!ctx || !cfg || n < 2 || n > 8 || N < 0 || N > HEGET_MAX_EVENTS || (N > 0 && !momenta)) return HEGET_EINVAL;
     if (cfg->mode < HEGET_GEN_FIXED || cfg->mode > HEGET_GEN_TOYPDF || !(cfg->a > 0.0)) return HEGET_EINVAL;
     if (cfg->mode == HEGET_GEN_LOGUNIFORM && !(cfg->b >= cfg->a)) return HEGET_EINVAL;
     DeviceGuard guard(ctx->device);
@@ -148,7 +148,7 @@ int heget_amp2_algo(heget_ctx* ctx, const double* momenta, int n, int precision,
                     int64_t N, void* stream)
 {
     if (algo < HEGET_ALGO_TREE || algo > HEGET_ALGO_TREE2) return HEGET_EINVAL;
-    if (!ctx || n < 2 || n > 8 || N < 0 || (N > 0 && (!momenta || !out_amp2))) return HEGET_EINVAL;
+    if (!ctx || n < 2 || n > 8 || N < 0 || N > HEGET_MAX_EVENTS || (N > 0 && (!momenta || !out_amp2))) return HEGET_EINVAL;
     if (precision != HEGET_FP32 && precision != HEGET_FP64) return HEGET_EINVAL;
     if ((reinterpret_cast<uintptr_t>(momenta) & 15u) != 0) return HEGET_EINVAL;
     DeviceGuard guard(ctx->device);
@@ -168,7 +168,7 @@ int heget_amp2_algo(heget_ctx* ctx, const double* momenta, int n, int precision,
 int heget_amp2_sampled(heget_ctx* ctx, uint64_t seed, uint64_t first_event, const double* momenta, int n,
                        int precision, double* out_amp2, int32_t* out_hel, int64_t N, void* stream)
 {
-    if (!ctx || n < 2 || n > 8 || N < 0 || (N > 0 && (!momenta || !out_amp2))) return HEGET_EINVAL;
+    if (!ctx || n < 2 || n > 8 || N < 0 || N > HEGET_MAX_EVENTS || (N > 0 && (!momenta || !out_amp2))) return HEGET_EINVAL;
     if (precision != HEGET_FP32 && precision != HEGET_FP64) return HEGET_EINVAL;
     if ((reinterpret_cast<uintptr_t>(momenta) & 15u) != 0) return HEGET_EINVAL;
     DeviceGuard guard(ctx->device);
@@ -183,7 +183,7 @@ int heget_amp2_sampled(heget_ctx* ctx, uint64_t seed, uint64_t first_event, cons
 int heget_list2(heget_ctx* ctx, uint64_t seed, uint64_t first_event, const double* momenta, int n, int precision,
                 double* out_amp2, int32_t* out_hel, int64_t N, void* stream)
 {
-    if (!ctx || n < 2 || n > 8 || N < 0 || (N > 0 && (!momenta || !out_amp2))) return HEGET_EINVAL;
+    if (!ctx || n < 2 || n > 8 || N < 0 || N > HEGET_MAX_EVENTS || (N > 0 && (!momenta || !out_amp2))) return HEGET_EINVAL;
     if (precision != HEGET_FP32 && precision != HEGET_FP64) return HEGET_EINVAL;
     DeviceGuard guard(ctx->device);
     if (!guard.ok) return fail_cuda(ctx, cudaGetLastError());
@@ -197,7 +197,7 @@ int heget_list2(heget_ctx* ctx, uint64_t seed, uint64_t first_event, const doubl
 int heget_list2_sum(heget_ctx* ctx, const double* momenta, int n, int precision, double* out_amp2, int64_t N,
                     void* stream)
 {
-    if (!ctx || n < 2 || n > 8 || N < 0 || (N > 0 && (!momenta || !out_amp2))) return HEGET_EINVAL;
+    if (!ctx || n < 2 || n > 8 || N < 0 || N > HEGET_MAX_EVENTS || (N > 0 && (!momenta || !out_amp2))) return HEGET_EINVAL;
     if (precision != HEGET_FP32 && precision != HEGET_FP64) return HEGET_EINVAL;
     DeviceGuard guard(ctx->device);
     if (!guard.ok) return fail_cuda(ctx, cudaGetLastError());
@@ -211,7 +211,7 @@ int heget_list2_sum(heget_ctx* ctx, const double* momenta, int n, int precision,
 int heget_histogram(heget_ctx* ctx, const double* momenta, const double* value, int n, int64_t N, int observable,
                     double lo, double hi, int nbins, double* hist, void* stream)
 {
-    if (!ctx || n < 2 || n > 8 || N < 0 || !hist || (N > 0 && (!momenta || !value))) return HEGET_EINVAL;
+    if (!ctx || n < 2 || n > 8 || N < 0 || N > HEGET_MAX_EVENTS || !hist || (N > 0 && (!momenta || !value))) return HEGET_EINVAL;
     if (observable < HEGET_OBS_PT_MAX || observable > HEGET_OBS_DR_ALL) return HEGET_EINVAL;
     if (nbins < 1 || nbins > HEGET_HIST_MAX_BINS || !(hi > lo)) return HEGET_EINVAL;
     if ((reinterpret_cast<uintptr_t>(momenta) & 15u) != 0) return HEGET_EINVAL;
@@ -227,7 +227,7 @@ int heget_histogram(heget_ctx* ctx, const double* momenta, const double* value, 
 int heget_helas_wavefunction(heget_ctx* ctx, int fn, int precision, const double* p, int nhel, int ns, double* w,
                                int64_t N, void* stream)
 {
-    if (!ctx || N < 0 || (N > 0 && (!p || !w))) return HEGET_EINVAL;
+    if (!ctx || N < 0 || N > HEGET_MAX_EVENTS || (N > 0 && (!p || !w))) return HEGET_EINVAL;
     if (fn < HEGET_FN_IXXXX0 || fn > HEGET_FN_VXXXX2) return HEGET_EINVAL;
     if (precision != HEGET_FP32 && precision != HEGET_FP64) return HEGET_EINVAL;
     if ((nhel != 1 && nhel != -1) || (ns != 1 && ns != -1)) return HEGET_EINVAL;
@@ -243,7 +243,7 @@ int heget_helas_wavefunction(heget_ctx* ctx, int fn, int precision, const double
 int heget_helas_vertex(heget_ctx* ctx, int fn, int precision, const double* fi, const double* fo, const double* vc,
                        double g, double* out, int64_t N, void* stream)
 {
-    if (!ctx || N < 0 || (N > 0 && !out)) return HEGET_EINVAL;
+    if (!ctx || N < 0 || N > HEGET_MAX_EVENTS || (N > 0 && !out)) return HEGET_EINVAL;
     if (fn < HEGET_VTX_IOVXXX || fn > HEGET_VTX_JIOXX0) return HEGET_EINVAL;
     if (precision != HEGET_FP32 && precision != HEGET_FP64) return HEGET_EINVAL;
     const bool need_fi = fn != HEGET_VTX_FVOXX0, need_fo = fn != HEGET_VTX_FVIXX0, need_vc = fn != HEGET_VTX_JIOXX0;
@@ -262,7 +262,7 @@ int heget_helas_vertex(heget_ctx* ctx, int fn, int precision, const double* fi, 
 int heget_xsec_reduce(heget_ctx* ctx, const double* amp2, const double* weight, int n, int64_t N, double* out3,
                       void* stream)
 {
-    if (!ctx || n < 2 || n > 8 || N < 0 || !out3 || (N > 0 && (!amp2 || !weight))) return HEGET_EINVAL;
+    if (!ctx || n < 2 || n > 8 || N < 0 || N > HEGET_MAX_EVENTS || !out3 || (N > 0 && (!amp2 || !weight))) return HEGET_EINVAL;
     DeviceGuard guard(ctx->device);
     if (!guard.ok) return fail_cuda(ctx, cudaGetLastError());
     int launches = 0;
@@ -274,7 +274,7 @@ int heget_xsec_reduce(heget_ctx* ctx, const double* amp2, const double* weight, 
 int heget_xsec_host(heget_ctx* ctx, const double* momenta, const double* weight, int n, int precision, int64_t N,
                     double* out_amp2, double* out3)
 {
-    if (!ctx || n < 2 || n > 8 || N < 0 || !out3 || (N > 0 && (!momenta || !weight))) return HEGET_EINVAL;
+    if (!ctx || n < 2 || n > 8 || N < 0 || N > HEGET_MAX_EVENTS || !out3 || (N > 0 && (!momenta || !weight))) return HEGET_EINVAL;
     if (precision != HEGET_FP32 && precision != HEGET_FP64) return HEGET_EINVAL;
     DeviceGuard guard(ctx->device);
     if (!guard.ok) return fail_cuda(ctx, cudaGetLastError());

@@ -81,6 +81,39 @@ def test_gen_events_empty(hg):
     assert m.shape == (0, 6, 4) and w.shape == (0,)
 
 
+def test_invalid_arguments_are_refused_before_any_launch(hg):
+    """include/heget.h, error behaviour: HEGET_EINVAL (-1) for n outside [2,8], N < 0 or above
+    HEGET_MAX_EVENTS, a bad precision / algorithm, null or misaligned buffers -- checked before the
+    buffers are touched, so the dummy pointers below are never dereferenced and nothing is launched."""
+    lib, ctx = hg._lib, hg._ctx
+    buf = torch.zeros(64, dtype=torch.float64, device=hg.device)
+    ptr = buf.data_ptr()
+    before = hg.launch_count()
+    bad = [
+        (ctx, ptr, 1, FP64, ptr, 1, None), (ctx, ptr, 9, FP64, ptr, 1, None),          # n
+        (ctx, ptr, 4, FP64, ptr, -1, None), (ctx, ptr, 4, FP64, ptr, 1 << 31, None),   # N
+        (ctx, ptr, 4, 2, ptr, 1, None),                                                # precision
+        (ctx, None, 4, FP64, ptr, 1, None), (ctx, ptr, 4, FP64, None, 1, None),        # null buffers
+        (ctx, ptr + 8, 4, FP64, ptr, 1, None),                                         # momenta not 16-byte aligned
+        (None, ptr, 4, FP64, ptr, 1, None),                                            # no context
+    ]
+    for args in bad:
+        assert lib.heget_amp2(*args) == -1, args
+    assert lib.heget_amp2_algo(ctx, ptr, 4, FP64, 3, ptr, 1, None) == -1
+    assert lib.heget_amp2_algo(ctx, ptr, 4, FP64, -1, ptr, 1, None) == -1
+    assert lib.heget_list2_sum(ctx, ptr, 4, FP64, ptr, 1 << 31, None) == -1
+    assert lib.heget_xsec_reduce(ctx, ptr, ptr, 4, 1 << 31, ptr, None) == -1
+    assert lib.heget_histogram(ctx, ptr, ptr, 4, 1, 0, 0.0, 1.0, 4095, ptr, None) == -1   # nbins > HEGET_HIST_MAX_BINS
+    assert lib.heget_histogram(ctx, ptr, ptr, 4, 1, 0, 1.0, 1.0, 8, ptr, None) == -1      # hi <= lo
+    assert hg.launch_count() == before
+    assert b"invalid argument" in lib.heget_strerror(-1)
+    # the largest accepted N is a property of the header: 2^31 - 1
+    hdr = open(__import__("os").path.join(__import__("os").path.dirname(__file__), "..", "include", "heget.h")).read()
+    assert "#define HEGET_MAX_EVENTS 2147483647LL" in hdr
+    assert lib.heget_amp2(ctx, ptr, 2, FP64, ptr, 0, None) == 0   # N = 0 is valid and launches nothing
+    assert hg.launch_count() == before
+
+
 @pytest.mark.parametrize("N", [0, 1, 255, 100003])
 def test_xsec_reduce_matches_oracle_and_is_deterministic(hg, N):
     rng = np.random.default_rng(N)
