@@ -39,14 +39,15 @@ def model_flops_per_event(n):
 def executed_flops_per_event(n, precision="fp32"):
     """What amp2_kernel executes: 2^n lanes (sigma_1 = +1 only, doubled by
     parity); per lane one fvixx0 node = 16 FMA + 4 MUL = 36 flop for every ordered prefix of up to
-    n-2 photons, and for each of the n!/2 prefixes of n-2 photons the two remaining orderings as
-    vertex + closing-table dot, 2 x (16 + 16) = 64 flop (the last fvixx0 + iovxxx of a branch
-    associated as <vbar|E'_b P . (E'_a psi)).  The fp64 4-photon kernel also computes the first two
-    tree levels once per event (48 two-node entries) instead of once per lane (16 nodes).  Tables
-    excluded.  Cross-checked against ncu's sass_thread_inst_executed_op_{f,d}{fma,mul,add} counters
-    in profiles/."""
+    n-2 photons, and for each of the n!/2 prefixes of n-2 photons the two remaining orderings as ONE
+    dot product with the pair closing table, 8 FMA = 16 flop (n >= 4; for n = 2, 3 as two
+    vertex + closing-table dots, 2 x (16 + 16) = 64 flop).  The fp64 4-photon kernel also computes
+    the first two tree levels once per event (48 two-node entries) instead of once per lane
+    (16 nodes).  Tables excluded.  Cross-checked against ncu's
+    sass_thread_inst_executed_op_{f,d}{fma,mul,add} counters in profiles/."""
     upper = sum(math.factorial(n) // math.factorial(n - l) for l in range(1, n - 1))
-    flops = 2 ** n * (36 * upper + 64 * (math.factorial(n) // 2))
+    closing = 16 if n >= 4 else 64
+    flops = 2 ** n * (36 * upper + closing * (math.factorial(n) // 2))
     if precision == "fp64" and n == 4:
         flops -= 2 ** n * 16 * 36 - 48 * 2 * 36
     return flops
@@ -366,12 +367,12 @@ def main():
                 "frac_note": "frac counts EXECUTED flops (what ncu counts); model_c_frac counts SURVEY 8(d)'s fixed "
                              "algorithmic figure (model C) over the same time.  Work removed by the parity relation and "
                              "by re-associating or sharing factors lowers frac while events/s and model_c_frac rise "
-                             "(4 gamma fp64: v3 1.48 ms, frac 0.56 -> v7 1.02 ms, frac 0.38)",
-                "flops_model": "executed: 2^n lanes x (36 flop per tree node down to depth n-2 + 64 per pair of last "
-                               "orderings), see executed_flops_per_event; model C (SURVEY 8(d)): 2*2^n x (44 per node "
+                             "(4 gamma fp64: v3 1.48 ms, frac 0.56 -> v7 1.02 ms, 0.48 -> v8 0.76 ms)",
+                "flops_model": "executed: 2^n lanes x (36 flop per tree node down to depth n-2 + 16 per pair of last "
+                               "orderings, one dot with the pair closing table), see executed_flops_per_event; model C (SURVEY 8(d)): 2*2^n x (44 per node "
                                "+ 24 per leaf), 3-5x the executed count because the kernel evaluates sigma_1=+1 only "
-                               "(parity), uses normalised polarisation blocks and contracts the last propagator into "
-                               "the closing vertex"}
+                               "(parity), uses normalised polarisation blocks and contracts the last two vertices and "
+                               "the last propagator of both final orderings into a per-event table"}
 
     result = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
               "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,

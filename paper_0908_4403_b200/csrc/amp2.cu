@@ -41,8 +41,14 @@ namespace {
                                // 3 gamma -6 %, 4 gamma +4 %, 5-7 gamma +-1 %: the shuffles cost the issue slots they save)
 #endif
 #ifndef HEGET_CLOSE
-#define HEGET_CLOSE 1   // last fvixx0 + iovxxx of a branch as vertex + closing-table dot (amp2_tree.cuh)
+#define HEGET_CLOSE 2   // 1: last fvixx0 + iovxxx of a branch as vertex + closing-table dot (amp2_tree.cuh, v7)
+                        // 2: the two orderings below a prefix of n-2 photons as ONE dot with the pair closing
+                        //    table (v8).  Measured on B200, 1 -> 2: 4 gamma 0.633 -> 0.549 ms fp32, 1.024 ->
+                        //    0.762 ms fp64; 8 gamma 841 -> 575 ms fp32, 1584 -> 951 ms fp64; 2 and 3 gamma
+                        //    4-14 % slower (the table costs more than it saves), so those stay on 1 (kClose)
 #endif
+template <int N>
+constexpr int kClose = (HEGET_CLOSE == 2 && N < 4) ? 1 : HEGET_CLOSE;
 #ifndef HEGET_SHARE64_MAXN
 #define HEGET_SHARE64_MAXN 7
 #endif
@@ -98,6 +104,8 @@ amp2_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_
     __shared__ double s_red[G::THREADS / 32];
     __shared__ double s_s2[G::EPB * N];  // s_i^2 = (pT/w)^2 taken out of photon i's E entries
     __shared__ Spinor<T> s_U[G::EPB * 2 * N];  // closing table (amp2_tree.cuh, close_weyl)
+    constexpr int NW = (kClose<N> == 2) ? 4 * (N * (N - 1) / 2) : 1;  // pair closing table entries per event
+    __shared__ Spinor<T> s_W[(kClose<N> == 2) ? G::EPB * NW : 1];
     constexpr int TOP = kTopShare<N, T> ? N * (N - 1) * 4 : 1;  // psi_2 entries per event
     __shared__ Spinor<T> s_top[kTopShare<N, T> ? G::EPB * TOP : 1];
 
@@ -114,7 +122,9 @@ amp2_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_
             if (batch + gridDim.x < n_batches) Tile::load(momenta, (batch + gridDim.x) * G::EPB, n_events, pf);
         }
         build_tables<N, T, G>(g, s_mom, s_P, s_E, s_s2);                        // a4, a5 (ends with a barrier)
-        if constexpr (HEGET_CLOSE != 0) build_closing_table<N, T, G>(s_P, s_E, s_U);
+        if constexpr (kClose<N> != 0) build_closing_table<N, T, G>(s_P, s_E, s_U);
+        if constexpr (kClose<N> == 2) build_pair_table<N, T, G>(s_U, s_E, s_W);
+        const Spinor<T>* closing = (kClose<N> == 2) ? s_W + ev_local * NW : s_U + ev_local * 2 * N;
 
         // a2, a6, a7: psi_0 = u(p1,+)/sqrt(2E1) = (1,0); walk the permutation tree
         T ar = 0, ai = 0;
@@ -136,11 +146,11 @@ amp2_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_
                 for (int jj = 0; jj < N - 1; ++jj) {
                     const int j = jj + (jj >= i ? 1 : 0);
                     const Spinor<T> f2 = top[(i * (N - 1) + jj) * 4 + 2 * ((hel >> i) & 1u) + ((hel >> j) & 1u)];
-                    Walk<N, 2, N - 2, T, kShare<N, T>, HEGET_CLOSE>::run(P, E, hel, (1u << i) | (1u << j), f2, ar, ai,
-                                                                        s_U + ev_local * 2 * N);
+                    Walk<N, 2, N - 2, T, kShare<N, T>, kClose<N>>::run(P, E, hel, (1u << i) | (1u << j), f2, ar, ai,
+                                                                        closing);
                 }
         } else {
-            Walk<N, 0, kBottom<N>, T, kShare<N, T>, HEGET_CLOSE>::run(P, E, hel, 0u, f0, ar, ai, s_U + ev_local * 2 * N);
+            Walk<N, 0, kBottom<N>, T, kShare<N, T>, kClose<N>>::run(P, E, hel, 0u, f0, ar, ai, closing);
         }
 
         // a8: |ampsum|^2 summed over the event's 2^N lanes, constant factors, store

@@ -131,6 +131,42 @@ __device__ __forceinline__ void build_closing_table(const PEntry<T>* s_P, const 
     __syncthreads();
 }
 
+// Pair closing table: the two orderings that share a prefix of n-2 photons end with (a, b) or
+// (b, a), and both close on the same spinor psi of that prefix:
+//   <vbar|E'_b P_{all\b} E'_a psi + <vbar|E'_a P_{all\a} E'_b psi = (U_b E'_a + U_a E'_b) . psi = W_ab . psi,
+// one row vector per unordered pair a < b and per helicity of a and b,
+//   W[4 (b(b-1)/2 + a) + 2 h_a + h_b],   (u0, u1) E' = (-u0 + a u1, -b u0 + u1).
+// Reads s_U and s_E (barrier before), ends with a barrier.
+template <typename T>
+__device__ __forceinline__ void accumulate_row_times_vertex(const Spinor<T>& u, const EEntry<T>& e, Spinor<T>& r)
+{
+    r.r0 += fma(e.ar, u.r1, fma(-e.ai, u.i1, -u.r0));
+    r.i0 += fma(e.ar, u.i1, fma(e.ai, u.r1, -u.i0));
+    r.r1 += fma(-e.br, u.r0, fma(e.bi, u.i0, u.r1));
+    r.i1 += fma(-e.br, u.i0, fma(-e.bi, u.r0, u.i1));
+}
+
+template <int N, typename T, typename G = Geometry<N>>
+__device__ __forceinline__ void build_pair_table(const Spinor<T>* s_U, const EEntry<T>* s_E, Spinor<T>* s_W)
+{
+    constexpr unsigned ITEMS = 4u * (N * (N - 1) / 2);
+    const int ev_local = threadIdx.x / G::L;
+    const unsigned lane = threadIdx.x % G::L;
+    const Spinor<T>* U = s_U + ev_local * 2 * N;
+    const EEntry<T>* E = s_E + ev_local * 2 * N;
+    for (unsigned q = lane; q < ITEMS; q += G::L) {
+        const unsigned pair = q >> 2, ha = (q >> 1) & 1u, hb = q & 1u;
+        unsigned b = 1;
+        while ((b + 1) * b / 2 <= pair) ++b;
+        const unsigned a = pair - b * (b - 1) / 2;
+        Spinor<T> w = {(T)0, (T)0, (T)0, (T)0};
+        accumulate_row_times_vertex(U[2 * b + hb], E[2 * a + ha], w);
+        accumulate_row_times_vertex(U[2 * a + ha], E[2 * b + hb], w);
+        s_W[ev_local * ITEMS + q] = w;
+    }
+    __syncthreads();
+}
+
 // a1 + a4 + a5 for the batch of events starting at ev0 (one-shot form).
 template <int N, typename T, typename G = Geometry<N>>
 __device__ __forceinline__ void build_event_tables(const double* __restrict__ momenta, int64_t ev0, int64_t n_events,

@@ -97,12 +97,22 @@ __device__ __forceinline__ EEntry<T> eselect(bool c, const EEntry<T>* a, const E
 // not helicity configurations), both nodes are computed.  hb[] = this lane's helicity bits.
 // CLOSE = 1: the last fvixx0 + iovxxx of every branch are evaluated as vertex + close_weyl with
 // the closing table (u[] = this lane's U entries of the remaining photons).
-template <int K, typename T, typename EA, int SHARE = 0, int CLOSE = 0>
+// CLOSE = 2: the last TWO orderings of every prefix of n-2 photons are one dot product with the
+// pair closing table (build_pair_table, amp2_common.cuh): idx[] = positions of the remaining
+// photons in the list Bottom<KB> started from, w[] = this lane's W entries of the KP = KB(KB-1)/2
+// pairs of that list (position pair p < q at q(q-1)/2 + p); u[] is unused.
+template <int K, typename T, typename EA, int SHARE = 0, int CLOSE = 0, int KP = 1>
 struct Bottom {
     static __device__ __forceinline__ void run(const PEntry<T>* __restrict__ PS, const int (&bit)[K],
                                                const EA (&e)[K], const unsigned (&hb)[K],
-                                               const Spinor<T>* const (&u)[K], const Spinor<T>& f, T& ar, T& ai)
+                                               const Spinor<T>* const (&u)[K], const int (&idx)[K],
+                                               const Spinor<T>* const (&w)[KP], const Spinor<T>& f, T& ar, T& ai)
     {
+        static_assert(!(SHARE == 1 && CLOSE == 2), "lane sharing and the pair table are alternatives");
+        if constexpr (K == 2 && CLOSE == 2) {
+            close_weyl(*w[idx[1] * (idx[1] - 1) / 2 + idx[0]], f, ar, ai);
+            return;
+        }
         if constexpr (K == 2 && CLOSE == 1) {
             if constexpr (SHARE == 1) {
                 if ((bit[0] | bit[1]) < 32) {  // uniform over the CTA
@@ -151,25 +161,28 @@ struct Bottom {
             EA sub_e[K - 1];
             unsigned sub_hb[K - 1];
             const Spinor<T>* sub_u[K - 1];
+            int sub_idx[K - 1];
 #pragma unroll
             for (int m = 0; m < K - 1; ++m) {
                 sub_bit[m] = bit[m + (m >= i ? 1 : 0)];
                 sub_e[m] = e[m + (m >= i ? 1 : 0)];
                 sub_hb[m] = hb[m + (m >= i ? 1 : 0)];
                 sub_u[m] = u[m + (m >= i ? 1 : 0)];
+                sub_idx[m] = idx[m + (m >= i ? 1 : 0)];
             }
             const PEntry<T>* Pn = PS + bit[i];
             const Spinor<T> fn = fvixx0_weyl(*Pn, eload<T>(e[i]), f);
-            Bottom<K - 1, T, EA, SHARE, CLOSE>::run(Pn, sub_bit, sub_e, sub_hb, sub_u, fn, ar, ai);
+            Bottom<K - 1, T, EA, SHARE, CLOSE, KP>::run(Pn, sub_bit, sub_e, sub_hb, sub_u, sub_idx, w, fn, ar, ai);
         }
     }
 };
 
-template <typename T, typename EA, int SHARE, int CLOSE>
-struct Bottom<1, T, EA, SHARE, CLOSE> {
+template <typename T, typename EA, int SHARE, int CLOSE, int KP>
+struct Bottom<1, T, EA, SHARE, CLOSE, KP> {
     static __device__ __forceinline__ void run(const PEntry<T>* __restrict__, const int (&)[1],
                                                const EA (&e)[1], const unsigned (&)[1],
-                                               const Spinor<T>* const (&)[1], const Spinor<T>& f, T& ar, T& ai)
+                                               const Spinor<T>* const (&)[1], const int (&)[1],
+                                               const Spinor<T>* const (&)[KP], const Spinor<T>& f, T& ar, T& ai)
     {
         iovxxx_weyl(eload<T>(e[0]), f, ar, ai);
     }
@@ -183,7 +196,7 @@ struct Walk {
                                                unsigned hel, unsigned used, const Spinor<T>& f, T& ar, T& ai,
                                                const Spinor<T>* __restrict__ U = nullptr)
     {
-        static_assert(CLOSE == 0 || KB >= 2, "the closing table replaces the last TWO levels");
+        static_assert(CLOSE == 0 || KB >= 2, "the closing tables replace the last TWO levels");
         unsigned avail = ((1u << N) - 1u) & ~used;
         if constexpr (N - DEPTH == KB) {
             int bit[KB];
@@ -194,19 +207,34 @@ struct Walk {
             using EA = std::conditional_t<BY_PTR, const EEntry<T>*, EEntry<T>>;
             EA e[KB];
             const Spinor<T>* u[KB];
+            int idx[KB], photon[KB];
 #pragma unroll
             for (int m = 0; m < KB; ++m) {
                 const int i = __ffs(avail) - 1;
                 avail &= avail - 1u;
                 bit[m] = 1 << i;
                 hb[m] = (hel >> i) & 1u;
-                u[m] = U + 2 * i + hb[m];
+                u[m] = (CLOSE == 2) ? nullptr : U + 2 * i + hb[m];
+                idx[m] = m;
+                photon[m] = i;
                 if constexpr (BY_PTR)
                     e[m] = &E[2 * i + hb[m]];
                 else
                     e[m] = E[2 * i + hb[m]];
             }
-            Bottom<KB, T, EA, SHARE, CLOSE>::run(P + used, bit, e, hb, u, f, ar, ai);
+            constexpr int KP = (CLOSE == 2) ? KB * (KB - 1) / 2 : 1;
+            const Spinor<T>* w[KP];
+            if constexpr (CLOSE == 2) {  // U is the pair closing table; photon[] is increasing
+#pragma unroll
+                for (int q = 1; q < KB; ++q)
+#pragma unroll
+                    for (int p = 0; p < q; ++p)
+                        w[q * (q - 1) / 2 + p] =
+                            U + 4 * (photon[q] * (photon[q] - 1) / 2 + photon[p]) + 2 * hb[p] + hb[q];
+            } else {
+                w[0] = nullptr;
+            }
+            Bottom<KB, T, EA, SHARE, CLOSE, KP>::run(P + used, bit, e, hb, u, idx, w, f, ar, ai);
         } else {
             while (avail) {
                 const int i = __ffs(avail) - 1;
