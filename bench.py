@@ -41,14 +41,14 @@ def executed_flops_per_event(n, precision="fp32"):
     parity); per lane one fvixx0 node = 16 FMA + 4 MUL = 36 flop for every ordered prefix of up to
     n-2 photons, and for each of the n!/2 prefixes of n-2 photons the two remaining orderings as ONE
     dot product with the pair closing table, 8 FMA = 16 flop (n >= 4; for n = 2, 3 as two
-    vertex + closing-table dots, 2 x (16 + 16) = 64 flop).  The fp64 4-photon kernel also computes
+    vertex + closing-table dots, 2 x (16 + 16) = 64 flop).  The 4-photon kernels also compute
     the first two tree levels once per event (48 two-node entries) instead of once per lane
     (16 nodes).  Tables excluded.  Cross-checked against ncu's
     sass_thread_inst_executed_op_{f,d}{fma,mul,add} counters in profiles/."""
     upper = sum(math.factorial(n) // math.factorial(n - l) for l in range(1, n - 1))
     closing = 16 if n >= 4 else 64
     flops = 2 ** n * (36 * upper + closing * (math.factorial(n) // 2))
-    if precision == "fp64" and n == 4:
+    if n == 4:
         flops -= 2 ** n * 16 * 36 - 48 * 2 * 36
     return flops
 

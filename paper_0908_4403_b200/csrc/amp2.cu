@@ -22,6 +22,10 @@
 #ifndef HEGET_MINW64
 #define HEGET_MINW64 (HEGET_MINB64 * 8)   // fp64: minimum resident warps per SM the register cap is set for
 #endif
+#ifndef HEGET_MINW64_N4
+#define HEGET_MINW64_N4 24                // ... of the 4-photon kernel (95 -> 80 registers: 0.768 -> 0.746 ms; for
+                                          // n >= 5 the same cap spills and is 15-30 % slower)
+#endif
 
 // CTA size of the tree kernels.  Small CTAs (64 threads: 4 events at n = 4) put more CTAs, each in
 // its own phase (load / tables / tree), on an SM at the same number of warps, which overlaps the
@@ -64,11 +68,15 @@ constexpr int kShare = (sizeof(T) == 8) ? ((N <= HEGET_SHARE64_MAXN) ? HEGET_SHA
 // the 2^N lanes of an event would each recompute the same N(N-1)*4 values (N = 4: 30 % of a
 // lane's tree).  With kTopShare the event's lanes compute each psi_2(i, j; h_i, h_j) once into
 // shared memory and every lane starts its N(N-1) subtrees from there.
-// Measured on B200 (2^20 events): 4 gamma fp64 1.350 -> 1.204 ms; 4 gamma fp32 unchanged; 5 gamma
-// slower in both precisions (the subtrees below depth 2 then start from three photons instead of
-// the four that Bottom<4> unrolls), so it is on for the fp64 4-photon kernel only.
+// Measured on B200 (2^20 events): 4 gamma fp64 1.350 -> 1.204 ms (v4); fp32 unchanged then, 0.554 ->
+// 0.526 ms since the pair closing table made the rest of the lane's tree cheap (v8); 5 gamma slower
+// in both precisions (the subtrees below depth 2 then start from three photons instead of the
+// four that Bottom<4> unrolls), so it is on for the 4-photon kernels only.
+#ifndef HEGET_TOPSHARE32
+#define HEGET_TOPSHARE32 1
+#endif
 template <int N, typename T>
-constexpr bool kTopShare = (N == 4 && sizeof(T) == 8);
+constexpr bool kTopShare = (N == 4 && (sizeof(T) == 8 || HEGET_TOPSHARE32 != 0));
 
 template <int N>
 constexpr int kBottom = (N < HEGET_KB) ? N : HEGET_KB;  // unrolled bottom levels of the tree
@@ -91,7 +99,8 @@ constexpr bool kPersistent = (HEGET_PERSIST32 != 0 && (sizeof(T) == 4) && (N == 
 
 template <int N, typename T>
 __global__ void __launch_bounds__(TreeGeometry<N>::THREADS,
-                                  ((sizeof(T) == 4) ? HEGET_MINB32 * 256 : HEGET_MINW64 * 32) / TreeGeometry<N>::THREADS)
+                                  ((sizeof(T) == 4) ? HEGET_MINB32 * 256 : (N == 4 ? HEGET_MINW64_N4 : HEGET_MINW64) * 32) /
+                                      TreeGeometry<N>::THREADS)
 amp2_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_t n_events, double g,
             int64_t n_batches)
 {

@@ -40,12 +40,15 @@ def test_flop_models_match_the_node_counts_of_the_survey():
         assert bench.model_flops_per_event(n) == 2 * 2 ** n * (44 * nodes + 24 * math.factorial(n))
         upper = nodes - math.factorial(n)            # prefixes of up to n-2 photons
         per_ordering = 8 if n >= 4 else 32          # pair closing table (n >= 4) / two vertex + dot closings
-        assert bench.executed_flops_per_event(n, "fp32") == 2 ** n * (36 * upper + per_ordering * math.factorial(n))
+        top_shared = (2 ** n * 16 - 48 * 2) * 36 if n == 4 else 0   # first two levels once per event
+        assert bench.executed_flops_per_event(n, "fp32") == (2 ** n * (36 * upper + per_ordering * math.factorial(n))
+                                                             - top_shared)
         assert bench.executed_flops_per_event(n, "fp64") <= bench.executed_flops_per_event(n, "fp32")
         for algo in ("subset", "two-sided"):
-            # never more work than the one-sided tree once there is a tree to speak of
+            # never more work than the one-sided tree once there is a tree to speak of (at n = 4 the
+            # tree kernel shares its first two levels between lanes and its tables are not counted)
             assert 0 < bench.executed_flops_per_event_algo(n, algo)
-            if n >= 4:
+            if n >= 5:
                 assert bench.executed_flops_per_event_algo(n, algo) <= bench.executed_flops_per_event(n, "fp32")
     # model C as tabulated in SURVEY 8(d): 1.09e3, 7.5e4, 2.06e9 flop per event
     assert abs(bench.model_flops_per_event(2) / 1.09e3 - 1) < 0.01
