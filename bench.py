@@ -25,7 +25,10 @@ if ROOT not in sys.path:
 METRIC = "events/s of summed |M|^2 for u ubar->n gamma"
 # dram__bytes_read.sum + dram__bytes_write.sum of one amp2 launch at the config's full size, from
 # the `ncu --set full` captures summarised under profiles/ (n, precision) -> bytes
-NCU_DRAM_BYTES = {(4, "fp64"): 211446528, (4, "fp32"): 210010112, (8, "fp64"): 21157888, (8, "fp32"): 21101824}
+NCU_DRAM_BYTES = {(4, "fp64"): 210962432, (4, "fp32"): 211015680, (8, "fp64"): 21132800, (8, "fp32"): 21054464}
+# flop per event of amp2_kernel as ncu counts them over the whole kernel, tables included
+# (smsp__sass_thread_inst_executed_op_{f,d}{fma x2, mul, add}_pred_on of the same captures / events)
+NCU_FLOPS_PER_EVENT = {(4, "fp64"): 9773.2, (4, "fp32"): 8788.5, (8, "fp64"): 349565175.5, (8, "fp32"): 349526649.8}
 UNIT = "events/s"
 
 
@@ -351,13 +354,20 @@ def main():
     peak_node = hg.fma_peak(prec, 2)
     sm_max = clocks["sm_max_mhz"] or 1965.0
     peak_theory = theoretical_peak(args.precision, torch.cuda.get_device_properties(local_rank).multi_processor_count, sm_max)
-    achieved = executed_flops_per_event_algo(n, args.algo, args.precision) * nl / (amp_ms * 1e-3)
+    tree_model = executed_flops_per_event_algo(n, args.algo, args.precision)
+    counted = NCU_FLOPS_PER_EVENT.get((n, args.precision)) if args.algo == "tree" else None
+    flops_per_event = counted if counted is not None else tree_model
+    achieved = flops_per_event * nl / (amp_ms * 1e-3)
     model_c = model_flops_per_event(n) * nl / (amp_ms * 1e-3)
     roofline = {"bound": "alu", "achieved": achieved / 1e12, "peak": peak_measured / 1e12, "unit": "TFLOP/s",
                 "frac": achieved / peak_measured, "traffic": NCU_DRAM_BYTES.get((n, args.precision)) if args.algo == "tree" else None,
                 "kernel": "%s<%d,%s>" % (KERNEL_NAME[args.algo], n, "double" if prec == FP64 else "float"),
                 "kernel_ms": amp_ms, "kernel_ms_best": amp_ms_best,
-                "flops_per_event_executed": executed_flops_per_event_algo(n, args.algo, args.precision),
+                "flops_per_event": flops_per_event,
+                "flops_source": ("ncu-counted over the whole kernel, tables included (profiles/)" if counted is not None
+                                 else "executed-instruction model of the tree, tables (< 1 % from 6 photons on) excluded"),
+                "flops_per_event_executed": tree_model,
+                "tree_model_tflops": tree_model * nl / (amp_ms * 1e-3) / 1e12,
                 "peak_source": "heget_fma_peak on this GPU: FMA with constant-bank operands "
                                "(MEASURED_PEAKS.json has no non-tensor figure)",
                 "peak_theoretical": peak_theory / 1e12, "frac_of_theoretical": achieved / peak_theory,
