@@ -55,7 +55,8 @@ amp2_sampled_kernel(const double* __restrict__ momenta, uint64_t seed, uint64_t 
     __shared__ PEntry<T> s_P[EPB * L];
     __shared__ EEntry<T> s_E[EPB * 2 * N];
     __shared__ double s_s2[EPB * N];
-    __shared__ Spinor<T> s_U[EPB * 2 * N];  // closing table (amp2_tree.cuh, close_weyl)
+    constexpr int NP = N * (N - 1) / 2;
+    __shared__ Spinor<T> s_W[EPB * NP];  // pair closing table of the drawn helicities (amp2_tree.cuh, CLOSE = 3)
 
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const int64_t ev0 = (int64_t)blockIdx.x * EPB;
@@ -83,8 +84,6 @@ amp2_sampled_kernel(const double* __restrict__ momenta, uint64_t seed, uint64_t 
             make_subset_entry<N, T>(mom, S, g, scale, &P[S]);
     }
     __syncthreads();
-    if (lane < 2 * N) s_U[w * 2 * N + lane] = closing_entry(E[lane], P[(L - 1) ^ (1 << (lane >> 1))]);
-    __syncthreads();
 
     const int64_t e = ev0 + w;
     const uint64_t gev = first_event + (uint64_t)(e < n_events ? e : n_events - 1);
@@ -94,6 +93,19 @@ amp2_sampled_kernel(const double* __restrict__ momenta, uint64_t seed, uint64_t 
     const bool s1 = bits & 1u, s2 = (bits >> 1) & 1u;
     const unsigned lam = (bits >> 2) & (unsigned)(L - 1);
     const unsigned hel = s1 ? lam : (~lam & (unsigned)(L - 1));   // parity image for sigma_1 = -1
+
+    // W_ab = U_b E'_a + U_a E'_b for the drawn helicities of a < b (build_pair_table, amp2_common.cuh)
+    if (lane < NP) {
+        unsigned b = 1;
+        while ((b + 1) * b / 2 <= (unsigned)lane) ++b;
+        const unsigned a = (unsigned)lane - b * (b - 1) / 2;
+        const EEntry<T> ea = E[2 * a + ((hel >> a) & 1u)], eb = E[2 * b + ((hel >> b) & 1u)];
+        Spinor<T> wab = {(T)0, (T)0, (T)0, (T)0};
+        accumulate_row_times_vertex(closing_entry(eb, P[(L - 1) ^ (1 << b)]), ea, wab);
+        accumulate_row_times_vertex(closing_entry(ea, P[(L - 1) ^ (1 << a)]), eb, wab);
+        s_W[w * NP + lane] = wab;
+    }
+    __syncthreads();
 
     T ar = 0, ai = 0;
     if (s1 != s2) {                                                // warp-uniform
@@ -110,7 +122,7 @@ amp2_sampled_kernel(const double* __restrict__ momenta, uint64_t seed, uint64_t 
                 used |= 1u << i;
                 f = fvixx0_weyl(P[used], E[2 * i + ((hel >> i) & 1u)], f);
             }
-            Walk<N, D, KB, T, 0, (KB >= 2) ? 1 : 0>::run(P, E, hel, used, f, ar, ai, s_U + w * 2 * N);
+            Walk<N, D, KB, T, 0, (KB >= 2) ? 3 : 0>::run(P, E, hel, used, f, ar, ai, s_W + w * NP);
         }
     }
     double dr = (double)ar, di = (double)ai;
@@ -144,6 +156,9 @@ amp2_sampled_kernel(const double* __restrict__ momenta, uint64_t seed, uint64_t 
 // deeper tree no longer fit the registers), so the switch is at N = 5.
 #ifndef HEGET_SAMPLED_THREAD_MAXN
 #define HEGET_SAMPLED_THREAD_MAXN 5
+#endif
+#ifndef HEGET_SAMPLED_PAIR_MINN
+#define HEGET_SAMPLED_PAIR_MINN 4   // thread kernel: pair closing table from this N on
 #endif
 
 template <int N, typename T>
@@ -188,12 +203,28 @@ amp2_sampled_thread_kernel(const double* __restrict__ momenta, uint64_t seed, ui
             else
                 make_subset_entry<N, T>(mom, S, g, scale, &P[S]);
         }
-        Spinor<T> U[2 * N];
-#pragma unroll
-        for (int q = 0; q < 2 * N; ++q) U[q] = closing_entry(E[q], P[(L - 1) ^ (1 << (q >> 1))]);
         T ar = 0, ai = 0;
         const Spinor<T> f0 = {(T)1, (T)0, (T)0, (T)0};
-        Walk<N, 0, N, T, 0, 1>::run(P, E, hel, 0u, f0, ar, ai, U);
+        if constexpr (N >= HEGET_SAMPLED_PAIR_MINN) {
+            // pair closing table of the drawn helicities (amp2_tree.cuh, CLOSE = 3)
+            Spinor<T> W[N * (N - 1) / 2];
+#pragma unroll
+            for (int b = 1; b < N; ++b)
+#pragma unroll
+                for (int a = 0; a < b; ++a) {
+                    const EEntry<T> ea = E[2 * a + ((hel >> a) & 1u)], eb = E[2 * b + ((hel >> b) & 1u)];
+                    Spinor<T> wab = {(T)0, (T)0, (T)0, (T)0};
+                    accumulate_row_times_vertex(closing_entry(eb, P[(L - 1) ^ (1 << b)]), ea, wab);
+                    accumulate_row_times_vertex(closing_entry(ea, P[(L - 1) ^ (1 << a)]), eb, wab);
+                    W[b * (b - 1) / 2 + a] = wab;
+                }
+            Walk<N, 0, N, T, 0, 3>::run(P, E, hel, 0u, f0, ar, ai, W);
+        } else {
+            Spinor<T> U[2 * N];
+#pragma unroll
+            for (int q = 0; q < 2 * N; ++q) U[q] = closing_entry(E[q], P[(L - 1) ^ (1 << (q >> 1))]);
+            Walk<N, 0, N, T, 0, 1>::run(P, E, hel, 0u, f0, ar, ai, U);
+        }
         if (sizeof(T) == 4) {
             const double inv = 1.0 / shat;
 #pragma unroll

@@ -100,7 +100,8 @@ __device__ __forceinline__ EEntry<T> eselect(bool c, const EEntry<T>* a, const E
 // CLOSE = 2: the last TWO orderings of every prefix of n-2 photons are one dot product with the
 // pair closing table (build_pair_table, amp2_common.cuh): idx[] = positions of the remaining
 // photons in the list Bottom<KB> started from, w[] = this lane's W entries of the KP = KB(KB-1)/2
-// pairs of that list (position pair p < q at q(q-1)/2 + p); u[] is unused.
+// pairs of that list (position pair p < q at q(q-1)/2 + p); u[] is unused.  CLOSE = 3: the same
+// with a table that holds ONE helicity assignment, W[b(b-1)/2 + a] (amp2_sampled.cu).
 template <int K, typename T, typename EA, int SHARE = 0, int CLOSE = 0, int KP = 1>
 struct Bottom {
     static __device__ __forceinline__ void run(const PEntry<T>* __restrict__ PS, const int (&bit)[K],
@@ -108,8 +109,8 @@ struct Bottom {
                                                const Spinor<T>* const (&u)[K], const int (&idx)[K],
                                                const Spinor<T>* const (&w)[KP], const Spinor<T>& f, T& ar, T& ai)
     {
-        static_assert(!(SHARE == 1 && CLOSE == 2), "lane sharing and the pair table are alternatives");
-        if constexpr (K == 2 && CLOSE == 2) {
+        static_assert(!(SHARE == 1 && CLOSE >= 2), "lane sharing and the pair table are alternatives");
+        if constexpr (K == 2 && CLOSE >= 2) {
             close_weyl(*w[idx[1] * (idx[1] - 1) / 2 + idx[0]], f, ar, ai);
             return;
         }
@@ -214,7 +215,7 @@ struct Walk {
                 avail &= avail - 1u;
                 bit[m] = 1 << i;
                 hb[m] = (hel >> i) & 1u;
-                u[m] = (CLOSE == 2) ? nullptr : U + 2 * i + hb[m];
+                u[m] = (CLOSE >= 2) ? nullptr : U + 2 * i + hb[m];
                 idx[m] = m;
                 photon[m] = i;
                 if constexpr (BY_PTR)
@@ -222,15 +223,16 @@ struct Walk {
                 else
                     e[m] = E[2 * i + hb[m]];
             }
-            constexpr int KP = (CLOSE == 2) ? KB * (KB - 1) / 2 : 1;
+            constexpr int KP = (CLOSE >= 2) ? KB * (KB - 1) / 2 : 1;
             const Spinor<T>* w[KP];
-            if constexpr (CLOSE == 2) {  // U is the pair closing table; photon[] is increasing
+            if constexpr (CLOSE >= 2) {  // U is the pair closing table; photon[] is increasing
 #pragma unroll
                 for (int q = 1; q < KB; ++q)
 #pragma unroll
-                    for (int p = 0; p < q; ++p)
-                        w[q * (q - 1) / 2 + p] =
-                            U + 4 * (photon[q] * (photon[q] - 1) / 2 + photon[p]) + 2 * hb[p] + hb[q];
+                    for (int p = 0; p < q; ++p) {
+                        const int pair = photon[q] * (photon[q] - 1) / 2 + photon[p];
+                        w[q * (q - 1) / 2 + p] = (CLOSE == 2) ? U + 4 * pair + 2 * hb[p] + hb[q] : U + pair;
+                    }
             } else {
                 w[0] = nullptr;
             }
