@@ -98,7 +98,9 @@ int heget_gen_events(heget_ctx* ctx, uint64_t seed, int n, const heget_gen_cfg* 
  * PAPER.md:435-439), the fvixx0 chain through the propagators (p1 - K_l)/t_l of eqs. (7),(8)
  * over all n! photon orderings of eq. (6), walked
  * as a depth-first permutation tree with every prefix computed once, closed by iovxxx
- * (PAPER.md:592-620), squared and summed over all 4*2^n helicities:
+ * (for n >= 4 the two orderings below a prefix of n-2 photons are closed
+ * together through a per-event table built from the ubar side), squared and
+ * summed over all 4*2^n helicities:
  *   out_amp2[e] = sum_{sigma1,sigma2,lambda_1..lambda_n} |M|^2   (the sum in eq. 2,
  *   PAPER.md:37, WITHOUT 1/(2 s_hat), spin/colour average and 1/n!).
  * precision selects the arithmetic of the tree walk (separate fp32 and fp64 kernels);
