@@ -12,6 +12,7 @@
 // Only sigma_1 = +1, sigma_2 = -1 is evaluated: sigma_1 = sigma_2 vanishes identically and
 // |M(-sigma,-lambda)| = |M(sigma,lambda)|, so the helicity sum is twice the sum over lambda.
 #include "amp2_tree.cuh"
+#include "amp2_chain.cuh"
 
 #ifndef HEGET_MINB32
 #define HEGET_MINB32 1      // __launch_bounds__ min CTAs per SM, fp32 / fp64 kernels
@@ -78,6 +79,18 @@ constexpr int kShare = (sizeof(T) == 8) ? ((N <= HEGET_SHARE64_MAXN) ? HEGET_SHA
 template <int N, typename T>
 constexpr bool kTopShare = (N == 4 && (sizeof(T) == 8 || HEGET_TOPSHARE32 != 0));
 
+// v9: factorised nodes psi = z v (amp2_chain.cuh) on top of the pair closing table.  Measured on
+// B200 see DESIGN.md section 6.1; n = 4 keeps the v8 form (its tree is 12 dots per lane on top of the
+// shared first two levels; the K table would cost more than it saves).
+#ifndef HEGET_CHAIN
+#define HEGET_CHAIN 1
+#endif
+#ifndef HEGET_CHAIN_MINN
+#define HEGET_CHAIN_MINN 5
+#endif
+template <int N>
+constexpr bool kChain = (HEGET_CHAIN != 0) && (kClose<N> == 2) && (N >= HEGET_CHAIN_MINN) && (N > HEGET_KB - 1) && (HEGET_KB >= 3);
+
 template <int N>
 constexpr int kBottom = (N < HEGET_KB) ? N : HEGET_KB;  // unrolled bottom levels of the tree
 
@@ -117,6 +130,8 @@ amp2_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_
     __shared__ Spinor<T> s_W[(kClose<N> == 2) ? G::EPB * NW : 1];
     constexpr int TOP = kTopShare<N, T> ? N * (N - 1) * 4 : 1;  // psi_2 entries per event
     __shared__ Spinor<T> s_top[kTopShare<N, T> ? G::EPB * TOP : 1];
+    constexpr int NK = kChain<N> ? (N * (N - 1) / 2) * N * 8 : 1;  // K table entries per event (amp2_chain.cuh)
+    __shared__ Cx<T> s_K[kChain<N> ? G::EPB * NK : 1];
 
     const int ev_local = threadIdx.x / G::L;
     const unsigned hel = threadIdx.x % G::L;
@@ -133,6 +148,7 @@ amp2_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_
         build_tables<N, T, G>(g, s_mom, s_P, s_E, s_s2);                        // a4, a5 (ends with a barrier)
         if constexpr (kClose<N> != 0) build_closing_table<N, T, G>(s_P, s_E, s_U);
         if constexpr (kClose<N> == 2) build_pair_table<N, T, G>(s_U, s_E, s_W);
+        if constexpr (kChain<N>) build_chain_table<N, T, G>(s_P, s_E, s_W, s_K);
         const Spinor<T>* closing = (kClose<N> == 2) ? s_W + ev_local * NW : s_U + ev_local * 2 * N;
 
         // a2, a6, a7: psi_0 = u(p1,+)/sqrt(2E1) = (1,0); walk the permutation tree
@@ -158,6 +174,9 @@ amp2_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_
                     Walk<N, 2, N - 2, T, kShare<N, T>, kClose<N>>::run(P, E, hel, (1u << i) | (1u << j), f2, ar, ai,
                                                                         closing);
                 }
+        } else if constexpr (kChain<N>) {
+            // the root is z = 1, v = (1, 0): rho = v_0 + b v_1 = 1 for every first photon
+            WalkChain<N, 0, kBottom<N>, T>::run(P, E, hel, 0u, (T)1, (T)0, f0, ar, ai, s_K + ev_local * NK);
         } else {
             Walk<N, 0, kBottom<N>, T, kShare<N, T>, kClose<N>>::run(P, E, hel, 0u, f0, ar, ai, closing);
         }
