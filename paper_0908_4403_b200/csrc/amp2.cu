@@ -88,6 +88,15 @@ constexpr bool kTopShare = (N == 4 && (sizeof(T) == 8 || HEGET_TOPSHARE32 != 0))
 #ifndef HEGET_CHAIN_MINN
 #define HEGET_CHAIN_MINN 5
 #endif
+#ifndef HEGET_CHAIN_KB32
+#define HEGET_CHAIN_KB32 4   // unrolled bottom levels of the factorised walk, fp32 / fp64
+#endif
+#ifndef HEGET_CHAIN_KB64
+#define HEGET_CHAIN_KB64 4
+#endif
+template <int N, typename T>
+constexpr int kChainBottom = (sizeof(T) == 4) ? ((N < HEGET_CHAIN_KB32) ? N : HEGET_CHAIN_KB32)
+                                              : ((N < HEGET_CHAIN_KB64) ? N : HEGET_CHAIN_KB64);
 template <int N>
 constexpr bool kChain = (HEGET_CHAIN != 0) && (kClose<N> == 2) && (N >= HEGET_CHAIN_MINN) && (N > HEGET_KB - 1) && (HEGET_KB >= 3);
 
@@ -175,8 +184,8 @@ amp2_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_
                                                                         closing);
                 }
         } else if constexpr (kChain<N>) {
-            // the root is z = 1, v = (1, 0): rho = v_0 + b v_1 = 1 for every first photon
-            WalkChain<N, 0, kBottom<N>, T>::run(P, E, hel, 0u, (T)1, (T)0, f0, ar, ai, s_K + ev_local * NK);
+            // the root is v = (1, 0): rho = v_0 + b v_1 = 1 for every first photon; ampsum = A(root)
+            WalkChain<N, 0, kChainBottom<N, T>, T>::run(P, E, hel, 0u, f0, ar, ai, s_K + ev_local * NK);
         } else {
             Walk<N, 0, kBottom<N>, T, kShare<N, T>, kClose<N>>::run(P, E, hel, 0u, f0, ar, ai, closing);
         }

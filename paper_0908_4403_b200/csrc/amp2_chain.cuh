@@ -16,8 +16,11 @@
 // its two remaining orderings with W_ab . psi = z (W_ab . v): the dot product depends on the event
 // only, so it is tabulated per event (build_chain_table),
 //     K[(pair(a,b) N + j) 8 + 4 h_j + 2 h_a + h_b] = W_ab(h_a,h_b) . v(all \ {a,b}, j, h_j),
-// and the closing is ampsum += z' K: 4 instructions instead of 8.  Per node: 14 instructions
-// (levels 1..n-3) or 12 (level n-2) instead of 20 and 28.
+// and the closing is z' K: 4 instructions instead of 8.  The walk does not carry z down: z is a
+// common factor of everything below a node, so each node RETURNS the sum of its subtree without it,
+//     A(node of n-2 photons) = K,   A(node) = sum over children j of rho_j A(child j),   ampsum = A(root)
+// (distributivity only; every ordering is still one term).  Per node: 14 instructions
+// (rho 4, v' 6, rho A 4; levels 1..n-3) or 8 (level n-2) instead of 20 and 28.
 #pragma once
 #include "amp2_common.cuh"
 
@@ -38,14 +41,20 @@ __device__ __forceinline__ Spinor<T> chain_vector(const PEntry<T>& P, const EEnt
     return v;
 }
 
-// z' = z (v_0 + b v_1)
+// rho = v_0 + b v_1
 template <typename T>
-__device__ __forceinline__ void chain_step(const Spinor<T>& v, const EEntry<T>& E, T zr, T zi, T& cr, T& ci)
+__device__ __forceinline__ void chain_rho(const Spinor<T>& v, const EEntry<T>& E, T& rr, T& ri)
 {
-    const T rr = fma(E.br, v.r1, fma(-E.bi, v.i1, v.r0));
-    const T ri = fma(E.br, v.i1, fma(E.bi, v.r1, v.i0));
-    cr = fma(zr, rr, -(zi * ri));
-    ci = fma(zr, ri, zi * rr);
+    rr = fma(E.br, v.r1, fma(-E.bi, v.i1, v.r0));
+    ri = fma(E.br, v.i1, fma(E.bi, v.r1, v.i0));
+}
+
+// s += rho a
+template <typename T>
+__device__ __forceinline__ void chain_acc(T rr, T ri, T xr, T xi, T& sr, T& si)
+{
+    sr = fma(rr, xr, fma(-ri, xi, sr));
+    si = fma(rr, xi, fma(ri, xr, si));
 }
 
 // Reads s_P, s_E and the pair closing table s_W (barrier before), ends with a barrier.
@@ -85,19 +94,19 @@ struct ChainBottom {
     static constexpr int KP = KB * (KB - 1) / 2;
     static __device__ __forceinline__ void run(const PEntry<T>* __restrict__ PS, const int (&bit)[K],
                                                const EEntry<T> (&e)[K], const int (&idx)[K],
-                                               const Cx<T>* const (&kp)[KP], const int (&jo)[KB], T zr, T zi,
+                                               const Cx<T>* const (&kp)[KP], const int (&jo)[KB],
                                                const Spinor<T>& v, T& ar, T& ai)
     {
         static_assert(K >= 3, "the K table closes the nodes of n-2 photons");
+        T sr = 0, si = 0;
 #pragma unroll
         for (int i = 0; i < K; ++i) {
-            T cr, ci;
-            chain_step(v, e[i], zr, zi, cr, ci);
+            T rr, ri;
+            chain_rho(v, e[i], rr, ri);
             if constexpr (K == 3) {
                 const int p = idx[i == 0 ? 1 : 0], q = idx[i == 2 ? 1 : 2];
                 const Cx<T> k = kp[q * (q - 1) / 2 + p][jo[idx[i]]];
-                ar = fma(cr, k.r, fma(-ci, k.i, ar));
-                ai = fma(cr, k.i, fma(ci, k.r, ai));
+                chain_acc(rr, ri, k.r, k.i, sr, si);
             } else {
                 int sub_bit[K - 1];
                 EEntry<T> sub_e[K - 1];
@@ -110,19 +119,24 @@ struct ChainBottom {
                 }
                 const PEntry<T>* Pn = PS + bit[i];
                 const Spinor<T> vc = chain_vector(*Pn, e[i]);
-                ChainBottom<K - 1, KB, T>::run(Pn, sub_bit, sub_e, sub_idx, kp, jo, cr, ci, vc, ar, ai);
+                T cr, ci;
+                ChainBottom<K - 1, KB, T>::run(Pn, sub_bit, sub_e, sub_idx, kp, jo, vc, cr, ci);
+                chain_acc(rr, ri, cr, ci, sr, si);
             }
         }
+        ar = sr;
+        ai = si;
     }
 };
 
-// Depth-first walk of the upper levels (`used` = photons already attached, uniform over the CTA);
+// Depth-first walk of the upper levels (`used` = photons already attached, uniform over the CTA;
+// returns A(node) in ar, ai);
 // when KB photons remain the unrolled ChainBottom<KB> takes over.  Needs N - KB >= 0 and KB >= 3.
 template <int N, int DEPTH, int KB, typename T>
 struct WalkChain {
     static __device__ __forceinline__ void run(const PEntry<T>* __restrict__ P, const EEntry<T>* __restrict__ E,
-                                               unsigned hel, unsigned used, T zr, T zi, const Spinor<T>& v, T& ar,
-                                               T& ai, const Cx<T>* __restrict__ Kt)
+                                               unsigned hel, unsigned used, const Spinor<T>& v, T& ar, T& ai,
+                                               const Cx<T>* __restrict__ Kt)
     {
         unsigned avail = ((1u << N) - 1u) & ~used;
         if constexpr (N - DEPTH == KB) {
@@ -149,18 +163,22 @@ struct WalkChain {
                     const int pair = photon[q] * (photon[q] - 1) / 2 + photon[p];
                     kp[q * (q - 1) / 2 + p] = Kt + pair * (N * 8) + 2 * hb[p] + hb[q];
                 }
-            ChainBottom<KB, KB, T>::run(P + used, bit, e, idx, kp, jo, zr, zi, v, ar, ai);
+            ChainBottom<KB, KB, T>::run(P + used, bit, e, idx, kp, jo, v, ar, ai);
         } else {
+            T sr = 0, si = 0;
             while (avail) {
                 const int i = __ffs(avail) - 1;
                 avail &= avail - 1u;
                 const unsigned S = used | (1u << i);
                 const EEntry<T> e = E[2 * i + ((hel >> i) & 1u)];
-                T cr, ci;
-                chain_step(v, e, zr, zi, cr, ci);
+                T rr, ri, cr, ci;
+                chain_rho(v, e, rr, ri);
                 const Spinor<T> vc = chain_vector(P[S], e);
-                WalkChain<N, DEPTH + 1, KB, T>::run(P, E, hel, S, cr, ci, vc, ar, ai, Kt);
+                WalkChain<N, DEPTH + 1, KB, T>::run(P, E, hel, S, vc, cr, ci, Kt);
+                chain_acc(rr, ri, cr, ci, sr, si);
             }
+            ar = sr;
+            ai = si;
         }
     }
 };
