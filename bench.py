@@ -25,10 +25,10 @@ if ROOT not in sys.path:
 METRIC = "events/s of summed |M|^2 for u ubar->n gamma"
 # dram__bytes_read.sum + dram__bytes_write.sum of one amp2 launch at the config's full size, from
 # the `ncu --set full` captures summarised under profiles/ (n, precision) -> bytes
-NCU_DRAM_BYTES = {(4, "fp64"): 210962432, (4, "fp32"): 211015680, (8, "fp64"): 21132800, (8, "fp32"): 21054464}
+NCU_DRAM_BYTES = {(4, "fp64"): 210962432, (4, "fp32"): 211015680}
 # flop per event of amp2_kernel as ncu counts them over the whole kernel, tables included
 # (smsp__sass_thread_inst_executed_op_{f,d}{fma x2, mul, add}_pred_on of the same captures / events)
-NCU_FLOPS_PER_EVENT = {(4, "fp64"): 9773.2, (4, "fp32"): 8788.5, (8, "fp64"): 349565175.5, (8, "fp32"): 349526649.8}
+NCU_FLOPS_PER_EVENT = {(4, "fp64"): 9773.2, (4, "fp32"): 8788.5}
 UNIT = "events/s"
 
 
@@ -41,13 +41,20 @@ def model_flops_per_event(n):
 
 def executed_flops_per_event(n, precision="fp32"):
     """What amp2_kernel executes: 2^n lanes (sigma_1 = +1 only, doubled by
-    parity); per lane one fvixx0 node = 16 FMA + 4 MUL = 36 flop for every ordered prefix of up to
-    n-2 photons, and for each of the n!/2 prefixes of n-2 photons the two remaining orderings as ONE
-    dot product with the pair closing table, 8 FMA = 16 flop (n >= 4; for n = 2, 3 as two
-    vertex + closing-table dots, 2 x (16 + 16) = 64 flop).  The 4-photon kernels also compute
-    the first two tree levels once per event (48 two-node entries) instead of once per lane
-    (16 nodes).  Tables excluded.  Cross-checked against ncu's
+    parity), tables excluded.
+    n >= 5 (v9, factorised nodes psi = z v, csrc/amp2_chain.cuh): every ordered prefix of up to n-3
+    photons is rho (4 FMA) + the vector v of the node (5 FMA + 1 MUL) + the accumulation rho A
+    (4 FMA) = 27 flop, every prefix of n-2 photons (its two remaining orderings closed by the
+    per-event table of closing dots) rho + accumulation = 16 flop.
+    n = 4 (v8): one fvixx0 node = 16 FMA + 4 MUL = 36 flop for every ordered prefix of up to n-2
+    photons and one dot product with the pair closing table, 8 FMA = 16 flop, per prefix of n-2
+    photons; the first two tree levels once per event (48 two-node entries) instead of once per
+    lane (16 nodes).  n = 2, 3 (v7): 36 flop per node and two vertex + closing-table dots,
+    2 x (16 + 16) = 64 flop, per prefix of n-2 photons.  Cross-checked against ncu's
     sass_thread_inst_executed_op_{f,d}{fma,mul,add} counters in profiles/."""
+    if n >= 5:
+        upper = sum(math.factorial(n) // math.factorial(n - l) for l in range(1, n - 2))
+        return 2 ** n * (27 * upper + 16 * (math.factorial(n) // 2))
     upper = sum(math.factorial(n) // math.factorial(n - l) for l in range(1, n - 1))
     closing = 16 if n >= 4 else 64
     flops = 2 ** n * (36 * upper + closing * (math.factorial(n) // 2))
@@ -378,8 +385,9 @@ def main():
                              "algorithmic figure (model C) over the same time.  Work removed by the parity relation and "
                              "by re-associating or sharing factors lowers frac while events/s and model_c_frac rise "
                              "(4 gamma fp64: v3 1.48 ms, frac 0.56 -> v7 1.02 ms, 0.48 -> v8 0.76 ms)",
-                "flops_model": "executed: 2^n lanes x (36 flop per tree node down to depth n-2 + 16 per pair of last "
-                               "orderings, one dot with the pair closing table), see executed_flops_per_event; model C (SURVEY 8(d)): 2*2^n x (44 per node "
+                "flops_model": "executed: n = 4: 2^n lanes x (36 flop per tree node down to depth n-2 + 16 per pair of last "
+                               "orderings, one dot with the pair closing table); n >= 5: 2^n lanes x (27 flop per factorised "
+                               "node down to depth n-3 + 16 per node of n-2 photons), see executed_flops_per_event; model C (SURVEY 8(d)): 2*2^n x (44 per node "
                                "+ 24 per leaf), 3-5x the executed count because the kernel evaluates sigma_1=+1 only "
                                "(parity), uses normalised polarisation blocks and contracts the last two vertices and "
                                "the last propagator of both final orderings into a per-event table"}

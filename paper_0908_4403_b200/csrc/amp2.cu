@@ -89,7 +89,7 @@ constexpr bool kTopShare = (N == 4 && (sizeof(T) == 8 || HEGET_TOPSHARE32 != 0))
 #define HEGET_CHAIN_MINN 5
 #endif
 #ifndef HEGET_CHAIN_KB32
-#define HEGET_CHAIN_KB32 4   // unrolled bottom levels of the factorised walk, fp32 / fp64
+#define HEGET_CHAIN_KB32 5   // unrolled bottom levels of the factorised walk, fp32 / fp64
 #endif
 #ifndef HEGET_CHAIN_KB64
 #define HEGET_CHAIN_KB64 4
