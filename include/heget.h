@@ -99,7 +99,9 @@ int heget_gen_events(heget_ctx* ctx, uint64_t seed, int n, const heget_gen_cfg* 
  * over all n! photon orderings of eq. (6), walked
  * as a depth-first permutation tree with every prefix computed once, closed by iovxxx
  * (for n >= 4 the two orderings below a prefix of n-2 photons are closed
- * together through a per-event table built from the ubar side), squared and
+ * together through a per-event table built from the ubar side; for n >= 5 each fvixx0 of the
+ * walk is evaluated in factorised form, a complex number times a per-(subset, photon) vector,
+ * which the rank-one polarisation blocks of massless photons allow), squared and
  * summed over all 4*2^n helicities:
  *   out_amp2[e] = sum_{sigma1,sigma2,lambda_1..lambda_n} |M|^2   (the sum in eq. 2,
  *   PAPER.md:37, WITHOUT 1/(2 s_hat), spin/colour average and 1/n!).
