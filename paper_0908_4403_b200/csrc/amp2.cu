@@ -23,8 +23,9 @@
 #ifndef HEGET_MINW64
 #define HEGET_MINW64 (HEGET_MINB64 * 8)   // fp64: minimum resident warps per SM the register cap is set for
 #endif
-#ifndef HEGET_MINW64_CHAIN
-#define HEGET_MINW64_CHAIN 24             // ... of the factorised (v9, n >= 5) kernels
+#ifndef HEGET_MINW64_N5
+#define HEGET_MINW64_N5 24                // ... of the 5-photon kernel (124 -> 78 registers, no spills: 5.02 -> 4.63 ms;
+                                          // the same cap leaves 6 gamma unchanged and costs 1-3 % at 7 and 8 gamma)
 #endif
 #ifndef HEGET_MINW64_N4
 #define HEGET_MINW64_N4 24                // ... of the 4-photon kernel (95 -> 80 registers: 0.768 -> 0.746 ms; for
@@ -124,7 +125,7 @@ constexpr bool kPersistent = (HEGET_PERSIST32 != 0 && (sizeof(T) == 4) && (N == 
 
 template <int N, typename T>
 __global__ void __launch_bounds__(TreeGeometry<N>::THREADS,
-                                  ((sizeof(T) == 4) ? HEGET_MINB32 * 256 : (N == 4 ? HEGET_MINW64_N4 : (N >= 5 ? HEGET_MINW64_CHAIN : HEGET_MINW64)) * 32) /
+                                  ((sizeof(T) == 4) ? HEGET_MINB32 * 256 : (N == 4 ? HEGET_MINW64_N4 : (N == 5 ? HEGET_MINW64_N5 : HEGET_MINW64)) * 32) /
                                       TreeGeometry<N>::THREADS)
 amp2_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_t n_events, double g,
             int64_t n_batches)

@@ -119,6 +119,30 @@ def test_polarisation_vectors_light_cone_gauge():
         assert abs(mdot(eps[(1, 1)], eps[(-1, 1)].conj())) < 1e-13
 
 
+def test_polarisation_slash_chiral_blocks_have_rank_one():
+    """eps-slash eps-slash = eps.eps = 0 for a circularly polarised massless photon, so each 2x2
+    chiral block of eps-slash (chiral representation, eq. 16 at PAPER.md:248) is singular: it is a
+    column times a row.  The factorised tree nodes of the CUDA path (v9) rest on
+    this property of vxxxx0 (eqs. 13-15); here it is checked on the oracle's
+    own polarisation vectors and gamma matrices."""
+    rng = np.random.default_rng(17)
+    metric = np.array([1.0, -1.0, -1.0, -1.0])
+    for _ in range(20):
+        v = rng.normal(size=3) * 80.0
+        p = np.array([np.linalg.norm(v), *v])
+        for lam in (-1, 1):
+            e = oracle.wavefunction("v", p, lam, 1)
+            slash = sum(metric[mu] * e[mu] * oracle.gamma(mu) for mu in range(4))
+            assert np.abs(slash @ slash).max() < 1e-13
+            upper, lower = slash[:2, 2:], slash[2:, :2]
+            assert np.abs(slash[:2, :2]).max() == 0 and np.abs(slash[2:, 2:]).max() == 0
+            for blk in (upper, lower):
+                scale = np.abs(blk).max() ** 2
+                assert scale > 1e-3                                   # the block itself is not zero
+                assert abs(np.linalg.det(blk)) < 1e-13 * max(scale, 1.0)
+                assert np.linalg.matrix_rank(blk, tol=1e-10) == 1
+
+
 def test_polarisation_vector_matches_paper_lists_9_and_10():
     # tests/golden/vxxxx_lists_9_10.txt: values printed in PAPER.md:553-559 (List 9, +z)
     # and 571-577 (List 10, -z); both lists are the nSV = -1 (initial-state) form.
