@@ -80,6 +80,9 @@ constexpr int kShare = (sizeof(T) == 8) ? ((N <= HEGET_SHARE64_MAXN) ? HEGET_SHA
 #ifndef HEGET_TOPSHARE32
 #define HEGET_TOPSHARE32 1
 #endif
+#ifndef HEGET_TOP_FACTORISED
+#define HEGET_TOP_FACTORISED 1
+#endif
 template <int N, typename T>
 constexpr bool kTopShare = (N == 4 && (sizeof(T) == 8 || HEGET_TOPSHARE32 != 0));
 
@@ -174,8 +177,23 @@ amp2_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_
             Spinor<T>* top = s_top + ev_local * TOP;
             for (int q = (int)hel; q < TOP; q += G::L) {
                 const int pair = q >> 2, i = pair / (N - 1), jj = pair % (N - 1), j = jj + (jj >= i ? 1 : 0);
+#if HEGET_TOP_FACTORISED
+                // factorised form (amp2_chain.cuh): psi_1 = v({i}, i), psi_2 = (v_0 + b_j v_1) v({i,j}, j),
+                // 24 instead of 40 instructions per entry
+                const EEntry<T> ej = E[2 * j + (q & 1)];
+                T rr, ri;
+                chain_rho(chain_vector(P[1u << i], E[2 * i + ((q >> 1) & 1)]), ej, rr, ri);
+                const Spinor<T> v2 = chain_vector(P[(1u << i) | (1u << j)], ej);
+                Spinor<T> f2;
+                f2.r0 = fma(rr, v2.r0, -(ri * v2.i0));
+                f2.i0 = fma(rr, v2.i0, ri * v2.r0);
+                f2.r1 = fma(rr, v2.r1, -(ri * v2.i1));
+                f2.i1 = fma(rr, v2.i1, ri * v2.r1);
+                top[q] = f2;
+#else
                 const Spinor<T> f1 = fvixx0_weyl(P[1u << i], E[2 * i + ((q >> 1) & 1)], f0);
                 top[q] = fvixx0_weyl(P[(1u << i) | (1u << j)], E[2 * j + (q & 1)], f1);
+#endif
             }
             __syncthreads();
 #pragma unroll

@@ -40,7 +40,7 @@ def test_flop_models_match_the_node_counts_of_the_survey():
         assert bench.model_flops_per_event(n) == 2 * 2 ** n * (44 * nodes + 24 * math.factorial(n))
         upper = nodes - math.factorial(n)            # prefixes of up to n-2 photons
         per_ordering = 8 if n >= 4 else 32          # pair closing table (n >= 4) / two vertex + dot closings
-        top_shared = (2 ** n * 16 - 48 * 2) * 36 if n == 4 else 0   # first two levels once per event
+        top_shared = (2 ** n * 16 * 36 - 48 * 42) if n == 4 else 0   # first two levels once per event, factorised entries
         if n >= 5:   # v9: factorised nodes, 27 flop down to n-3 photons, 16 per node of n-2 photons
             deep = math.factorial(n) // 2               # prefixes of exactly n-2 photons
             expect = 2 ** n * (27 * (upper - deep) + 16 * deep)
