@@ -1,14 +1,16 @@
 // amp2.cu -- heget_amp2: summed squared helicity amplitude of u ubar -> n gamma (product code).
 //
-// Mapping: one lane per photon-helicity configuration (2^N lanes per event), 256-thread CTAs
-// holding 256/2^N events.  All lanes of a CTA walk the SAME permutation tree in lockstep
+// Mapping: one lane per photon-helicity configuration (2^N lanes per event), CTAs of
+// max(64, 2^N) threads holding 64/2^N events (one event from n = 6 on).  All lanes of a CTA walk the SAME permutation tree in lockstep
 // (no divergence); they differ only in which helicity entry of the per-photon E table they
 // read.  Per event the CTA first builds, in shared memory,
 //   - the E table (vxxxx0 for both helicities of every photon) and
 //   - the subset table P[S] = -g/t_S * (p1 - K_S)-slash block for every photon subset S,
 // then every lane runs the depth-first walk of eq. (6)'s n! orderings: each
 // ordered prefix (tree node) is one fvixx0 computed once, each leaf one
-// iovxxx accumulated into ampsum (List 2).
+// iovxxx accumulated into ampsum (List 2).  For n >= 4 the two
+// orderings below a prefix of n-2 photons close through a per-event pair table (amp2_common.cuh);
+// for n >= 5 the nodes are evaluated in factorised form psi = z v (amp2_chain.cuh).
 // Only sigma_1 = +1, sigma_2 = -1 is evaluated: sigma_1 = sigma_2 vanishes identically and
 // |M(-sigma,-lambda)| = |M(sigma,lambda)|, so the helicity sum is twice the sum over lambda.
 #include "amp2_tree.cuh"

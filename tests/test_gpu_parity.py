@@ -122,7 +122,7 @@ def test_amp2_two_photon_closed_form_fixed_energy(hg, algo):
     assert np.all(rel32 <= TOL32)
 
 
-@pytest.mark.parametrize("n", [2, 4, 7])
+@pytest.mark.parametrize("n", [2, 4, 5, 6, 7])
 @pytest.mark.parametrize("algo", ALGOS)
 def test_amp2_edge_sizes(hg, n, algo):
     mom, _ = oracle.gen_events(9, n, 3, mode=oracle.MODE_FIXED, a=800.0)
@@ -149,6 +149,22 @@ def test_amp2_is_deterministic_and_batch_independent(hg, algo):
     assert np.array_equal(a, b)
     c = gpu_amp2(hg, mom[123:777], FP64, algo)     # different CTA alignment, same per-event result
     assert np.array_equal(a[123:777], c)
+
+
+@pytest.mark.parametrize("n", [5, 6, 7])
+@pytest.mark.parametrize("precision", [FP64, FP32])
+def test_factorised_tree_kernels_are_deterministic_and_alignment_independent(hg, n, precision):
+    """The n >= 5 tree kernels (factorised nodes, per-event table of closing dots; DESIGN.md 6.1 v9)
+    hold one or two events per CTA: the per-event result must not depend on which CTA slot an
+    event lands in, on its neighbours, or on the run."""
+    c = workloads.CONFIGS["4gamma"]
+    mom, _ = oracle.gen_events(c["seed"], n, 301, mode=c["mode"], a=c["a"], b=c["b"], y_max=c["y_max"],
+                               apply_cuts=True)
+    a = gpu_amp2(hg, mom, precision)
+    assert np.array_equal(a, gpu_amp2(hg, mom, precision))
+    assert np.array_equal(a[37:290], gpu_amp2(hg, mom[37:290], precision))
+    assert np.array_equal(a[300:], gpu_amp2(hg, mom[300:], precision))
+    assert np.all(np.isfinite(a)) and np.all(a > 0)
 
 
 def test_invalid_arguments_return_einval(hg):
