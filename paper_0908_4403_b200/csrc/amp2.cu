@@ -82,6 +82,9 @@ constexpr int kShare = (sizeof(T) == 8) ? ((N <= HEGET_SHARE64_MAXN) ? HEGET_SHA
 #ifndef HEGET_TOPSHARE32
 #define HEGET_TOPSHARE32 1
 #endif
+#ifndef HEGET_PAIR_DIRECT
+#define HEGET_PAIR_DIRECT 1   // pair closing table in one phase (build_pair_table_direct, amp2_common.cuh)
+#endif
 #ifndef HEGET_TOP_FACTORISED
 #define HEGET_TOP_FACTORISED 1
 #endif
@@ -143,7 +146,7 @@ amp2_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_
     __shared__ EEntry<T> s_E[G::EPB * 2 * N];
     __shared__ double s_red[G::THREADS / 32];
     __shared__ double s_s2[G::EPB * N];  // s_i^2 = (pT/w)^2 taken out of photon i's E entries
-    __shared__ Spinor<T> s_U[G::EPB * 2 * N];  // closing table (amp2_tree.cuh, close_weyl)
+    __shared__ Spinor<T> s_U[(kClose<N> == 2 && HEGET_PAIR_DIRECT != 0) ? 1 : G::EPB * 2 * N];  // closing table (amp2_tree.cuh, close_weyl)
     constexpr int NW = (kClose<N> == 2) ? 4 * (N * (N - 1) / 2) : 1;  // pair closing table entries per event
     __shared__ Spinor<T> s_W[(kClose<N> == 2) ? G::EPB * NW : 1];
     constexpr int TOP = kTopShare<N, T> ? N * (N - 1) * 4 : 1;  // psi_2 entries per event
@@ -164,8 +167,13 @@ amp2_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_
             if (batch + gridDim.x < n_batches) Tile::load(momenta, (batch + gridDim.x) * G::EPB, n_events, pf);
         }
         build_tables<N, T, G>(g, s_mom, s_P, s_E, s_s2);                        // a4, a5 (ends with a barrier)
-        if constexpr (kClose<N> != 0) build_closing_table<N, T, G>(s_P, s_E, s_U);
-        if constexpr (kClose<N> == 2) build_pair_table<N, T, G>(s_U, s_E, s_W);
+        if constexpr (kClose<N> == 2 && HEGET_PAIR_DIRECT != 0) {
+            // W straight from P and E; with kTopShare the barrier is the one after the top table below
+            build_pair_table_direct<N, T, G, !kTopShare<N, T>>(s_P, s_E, s_W);
+        } else {
+            if constexpr (kClose<N> != 0) build_closing_table<N, T, G>(s_P, s_E, s_U);
+            if constexpr (kClose<N> == 2) build_pair_table<N, T, G>(s_U, s_E, s_W);
+        }
         if constexpr (kChain<N>) build_chain_table<N, T, G>(s_P, s_E, s_W, s_K);
         const Spinor<T>* closing = (kClose<N> == 2) ? s_W + ev_local * NW : s_U + ev_local * 2 * N;
 

@@ -167,6 +167,32 @@ __device__ __forceinline__ void build_pair_table(const Spinor<T>* s_U, const EEn
     __syncthreads();
 }
 
+// The same table straight from the P and E tables (the closing entries U_a, U_b of an item are
+// evaluated in place, bit-identical to the two-step form): one phase and one barrier less, which
+// is what counts in the latency-bound small-n kernels.  SYNC = false leaves the barrier to the
+// caller (amp2.cu fills the shared first two tree levels in the same phase).
+template <int N, typename T, typename G = Geometry<N>, bool SYNC = true>
+__device__ __forceinline__ void build_pair_table_direct(const PEntry<T>* s_P, const EEntry<T>* s_E, Spinor<T>* s_W)
+{
+    constexpr unsigned ITEMS = 4u * (N * (N - 1) / 2);
+    const int ev_local = threadIdx.x / G::L;
+    const unsigned lane = threadIdx.x % G::L;
+    const PEntry<T>* P = s_P + ev_local * G::L;
+    const EEntry<T>* E = s_E + ev_local * 2 * N;
+    for (unsigned q = lane; q < ITEMS; q += G::L) {
+        const unsigned pair = q >> 2, ha = (q >> 1) & 1u, hb = q & 1u;
+        unsigned b = 1;
+        while ((b + 1) * b / 2 <= pair) ++b;
+        const unsigned a = pair - b * (b - 1) / 2;
+        const EEntry<T> ea = E[2 * a + ha], eb = E[2 * b + hb];
+        Spinor<T> w = {(T)0, (T)0, (T)0, (T)0};
+        accumulate_row_times_vertex(closing_entry(eb, P[(G::L - 1) ^ (1u << b)]), ea, w);
+        accumulate_row_times_vertex(closing_entry(ea, P[(G::L - 1) ^ (1u << a)]), eb, w);
+        s_W[ev_local * ITEMS + q] = w;
+    }
+    if constexpr (SYNC) __syncthreads();
+}
+
 // a1 + a4 + a5 for the batch of events starting at ev0 (one-shot form).
 template <int N, typename T, typename G = Geometry<N>>
 __device__ __forceinline__ void build_event_tables(const double* __restrict__ momenta, int64_t ev0, int64_t n_events,
