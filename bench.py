@@ -25,7 +25,7 @@ if ROOT not in sys.path:
 METRIC = "events/s of summed |M|^2 for u ubar->n gamma"
 # dram__bytes_read.sum + dram__bytes_write.sum of one amp2 launch at the config's full size, from
 # the `ncu --set full` captures summarised under profiles/ (n, precision) -> bytes
-NCU_DRAM_BYTES = {(4, "fp64"): 210792192, (4, "fp32"): 212225536, (8, "fp64"): 21108480, (8, "fp32"): 21051648}
+NCU_DRAM_BYTES = {(4, "fp64"): 210208512, (4, "fp32"): 210454784, (8, "fp64"): 21108480, (8, "fp32"): 21051648}
 # flop per event of amp2_kernel as ncu counts them over the whole kernel, tables included
 # (smsp__sass_thread_inst_executed_op_{f,d}{fma x2, mul, add}_pred_on of the same captures / events)
 NCU_FLOPS_PER_EVENT = {(4, "fp64"): 8815.0, (4, "fp32"): 7865.1, (8, "fp64"): 1.4349e8, (8, "fp32"): 1.4346e8}
@@ -384,7 +384,7 @@ def main():
                 "frac_note": "frac counts EXECUTED flops (what ncu counts); model_c_frac counts SURVEY 8(d)'s fixed "
                              "algorithmic figure (model C) over the same time.  Work removed by the parity relation and "
                              "by re-associating or sharing factors lowers frac while events/s and model_c_frac rise "
-                             "(4 gamma fp64: v3 1.48 ms, frac 0.56 -> v7 1.02 ms, 0.48 -> v8 0.745 ms, 0.41 -> v9 0.713 ms, 0.39)",
+                             "(4 gamma fp64: v3 1.48 ms, frac 0.56 -> v7 1.02 ms, 0.48 -> v8 0.745 ms, 0.41 -> v9 0.70 ms, 0.39)",
                 "flops_model": "executed: n = 4: 2^n lanes x (36 flop per tree node down to depth n-2 + 16 per pair of last "
                                "orderings, one dot with the pair closing table); n >= 5: 2^n lanes x (27 flop per factorised "
                                "node down to depth n-3 + 16 per node of n-2 photons), see executed_flops_per_event; model C (SURVEY 8(d)): 2*2^n x (44 per node "

@@ -30,8 +30,9 @@
                                           // the same cap leaves 6 gamma unchanged and costs 1-3 % at 7 and 8 gamma)
 #endif
 #ifndef HEGET_MINW64_N4
-#define HEGET_MINW64_N4 24                // ... of the 4-photon kernel (95 -> 80 registers: 0.768 -> 0.746 ms; for
-                                          // n >= 5 the same cap spills and is 15-30 % slower)
+#define HEGET_MINW64_N4 32                // ... of the 4-photon kernel (95 -> 80 registers: 0.768 -> 0.746 ms in v8; v9 with
+                                          // the one-phase pair table: 80 -> 72 -> 64 registers, no spills, 16 CTAs per SM:
+                                          // 0.713 -> 0.704 -> 0.701 ms; for n >= 6 such caps spill and are 15-30 % slower)
 #endif
 
 // CTA size of the tree kernels.  Small CTAs (64 threads: 4 events at n = 4) put more CTAs, each in
