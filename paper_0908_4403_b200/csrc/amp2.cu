@@ -25,6 +25,11 @@
 #ifndef HEGET_MINW64
 #define HEGET_MINW64 (HEGET_MINB64 * 8)   // fp64: minimum resident warps per SM the register cap is set for
 #endif
+#ifndef HEGET_MINW32_N4
+#define HEGET_MINW32_N4 8                 // fp32 4-photon kernel: minimum resident warps per SM; 8 = no cap (110 registers).
+                                          // Measured: 24 (80 registers) 0.521 ms, 32 (64 registers) 0.525 ms against 0.502 ms
+                                          // uncapped (no spills in any of them): the persistent fp32 kernel prefers registers
+#endif
 #ifndef HEGET_MINW64_N5
 #define HEGET_MINW64_N5 24                // ... of the 5-photon kernel (124 -> 78 registers, no spills: 5.02 -> 4.63 ms;
                                           // the same cap leaves 6 gamma unchanged and costs 1-3 % at 7 and 8 gamma)
@@ -134,7 +139,7 @@ constexpr bool kPersistent = (HEGET_PERSIST32 != 0 && (sizeof(T) == 4) && (N == 
 
 template <int N, typename T>
 __global__ void __launch_bounds__(TreeGeometry<N>::THREADS,
-                                  ((sizeof(T) == 4) ? HEGET_MINB32 * 256 : (N == 4 ? HEGET_MINW64_N4 : (N == 5 ? HEGET_MINW64_N5 : HEGET_MINW64)) * 32) /
+                                  ((sizeof(T) == 4) ? ((N == 4) ? HEGET_MINW32_N4 * 32 : HEGET_MINB32 * 256) : (N == 4 ? HEGET_MINW64_N4 : (N == 5 ? HEGET_MINW64_N5 : HEGET_MINW64)) * 32) /
                                       TreeGeometry<N>::THREADS)
 amp2_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_t n_events, double g,
             int64_t n_batches)
