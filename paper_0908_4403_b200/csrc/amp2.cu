@@ -20,7 +20,7 @@
 #define HEGET_MINB32 1      // __launch_bounds__ min CTAs per SM, fp32 / fp64 kernels
 #endif
 #ifndef HEGET_MINB64
-#define HEGET_MINB64 2
+#define HEGET_MINB64 1
 #endif
 #ifndef HEGET_MINW64
 #define HEGET_MINW64 (HEGET_MINB64 * 8)   // fp64: minimum resident warps per SM the register cap is set for
@@ -110,11 +110,14 @@ constexpr bool kTopShare = (N == 4 && (sizeof(T) == 8 || HEGET_TOPSHARE32 != 0))
 #define HEGET_CHAIN_KB32 5   // unrolled bottom levels of the factorised walk, fp32 / fp64
 #endif
 #ifndef HEGET_CHAIN_KB64
-#define HEGET_CHAIN_KB64 4
+#define HEGET_CHAIN_KB64 5   // n >= 6, with the register cap lifted (HEGET_MINB64 = 1: 160-185 registers, 8-12 warps per
+                             // SM, no spills).  Measured against four levels under the 128-register cap (16 warps):
+                             // 6 gamma 34.1 -> 29.5 ms, 7 gamma 110.8 -> 96.6 ms, 8 gamma 440 -> 375 ms; five levels
+                             // UNDER the cap spill 800 B
 #endif
 template <int N, typename T>
 constexpr int kChainBottom = (sizeof(T) == 4) ? ((N < HEGET_CHAIN_KB32) ? N : HEGET_CHAIN_KB32)
-                                              : ((N < HEGET_CHAIN_KB64) ? N : HEGET_CHAIN_KB64);
+                                              : ((N < 6) ? ((N < 4) ? N : 4) : HEGET_CHAIN_KB64);  // 5 gamma: capped at 80 registers
 template <int N>
 constexpr bool kChain = (HEGET_CHAIN != 0) && (kClose<N> == 2) && (N >= HEGET_CHAIN_MINN) && (N > HEGET_KB - 1) && (HEGET_KB >= 3);
 
