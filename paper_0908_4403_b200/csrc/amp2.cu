@@ -20,7 +20,9 @@
 #define HEGET_MINB32 1      // __launch_bounds__ min CTAs per SM, fp32 / fp64 kernels
 #endif
 #ifndef HEGET_MINB64
-#define HEGET_MINB64 1
+#define HEGET_MINB64 1      // fp64 (n = 2, 3 and n >= 6): 1 = no register cap.  The v2-v8 tree kernels ran best at 2
+                            // (128 registers, 16 warps per SM); the factorised walk with five unrolled levels
+                            // (HEGET_CHAIN_KB64) needs 160-185 registers and is 13-15 % faster uncapped
 #endif
 #ifndef HEGET_MINW64
 #define HEGET_MINW64 (HEGET_MINB64 * 8)   // fp64: minimum resident warps per SM the register cap is set for
