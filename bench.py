@@ -25,7 +25,7 @@ if ROOT not in sys.path:
 METRIC = "events/s of summed |M|^2 for u ubar->n gamma"
 # dram__bytes_read.sum + dram__bytes_write.sum of one amp2 launch at the config's full size, from
 # the `ncu --set full` captures summarised under profiles/ (n, precision) -> bytes
-NCU_DRAM_BYTES = {(4, "fp64"): 210208512, (4, "fp32"): 210454784, (8, "fp64"): 21108480, (8, "fp32"): 21051648}
+NCU_DRAM_BYTES = {(4, "fp64"): 210208512, (4, "fp32"): 210454784, (8, "fp64"): 21140480, (8, "fp32"): 21051648}
 # flop per event of amp2_kernel as ncu counts them over the whole kernel, tables included
 # (smsp__sass_thread_inst_executed_op_{f,d}{fma x2, mul, add}_pred_on of the same captures / events)
 NCU_FLOPS_PER_EVENT = {(4, "fp64"): 8815.0, (4, "fp32"): 7865.1, (8, "fp64"): 1.4349e8, (8, "fp32"): 1.4346e8}
