@@ -14,8 +14,12 @@
  *  - [dev] calls are asynchronous on `stream` (a cudaStream_t passed as void*, NULL = the
  *    legacy default stream) and do not synchronise the host; *_host calls return after
  *    the result is in the host buffer;
- *  - a context is not thread-safe: calls on the SAME heget_ctx must not overlap in time
- *    (different contexts, e.g. one per GPU or per host thread, are independent);
+ *  - a context is not thread-safe: host calls on the SAME heget_ctx must not overlap in time
+ *    (different contexts, e.g. one per GPU or per host thread, are independent).  [dev] calls
+ *    of one context may be issued on DIFFERENT streams and run concurrently; the only scratch a
+ *    [dev] call uses is heget_xsec_reduce's block partials, a ring of HEGET_REDUCE_SLOTS
+ *    buffers used round-robin, so at most HEGET_REDUCE_SLOTS reductions of one context may be
+ *    in flight at the same time (heget_xsec_host has staging and partials of its own);
  *  - momenta layout: double[N][n+2][4], four-vectors (E,px,py,pz) (PAPER.md:474-477,
  *    553-554), particle order u, ubar, gamma_1..gamma_n (p1..p5 of List 2);
  *    the base pointer must be 16-byte aligned.
@@ -49,6 +53,9 @@ enum {
  * at 32 (n + 2) bytes of momenta per event such a batch does not fit one B200 anyway. */
 #define HEGET_MAX_EVENTS 2147483647LL
 
+/* heget_xsec_reduce calls of one context that may be in flight on different streams at once. */
+#define HEGET_REDUCE_SLOTS 8
+
 /* Event-generation modes of heget_gen_events ("input recipe"). */
 enum {
     HEGET_GEN_FIXED = 0,      /* sqrt_s_hat = a, y = 0 */
@@ -67,7 +74,8 @@ typedef struct heget_gen_cfg {
 /* Create a context on CUDA device `device`.
  *   alpha, q_charge : fine-structure constant and quark charge; the FFV coupling is
  *                     gal[0] = gal[1] = -e Q_q, e = sqrt(4 pi alpha) (eq. 26)
- *   pt_cut, eta_cut, dr_cut : final-state cuts of eq. (9)
+ *   pt_cut, eta_cut, dr_cut : final-state cuts of eq. (9); finite and >= 0
+ * alpha <= 0 or a non-finite argument gives HEGET_EINVAL.
  * *out is written on success only and must be released with heget_destroy. */
 int heget_init(int device, double alpha, double q_charge, double pt_cut, double eta_cut,
                double dr_cut, heget_ctx** out);
@@ -89,6 +97,8 @@ int heget_rambo(heget_ctx* ctx, uint64_t seed, int n, double sqrt_s_hat, int64_t
  *   w = [cuts] * Phi_n(s_hat) / (2 s_hat) * (TOYPDF: Jacobian * 2 f(x1) f(x2))
  * (eqs. 1-4).  Global event index = first_event + local index, so any
  * contiguous shard of a run reproduces the same events (multi-GPU: shard by index range).
+ * HEGET_GEN_TOYPDF needs tau_min = (n pt_cut)^2 / a^2 inside (0, 1) (the context's pt_cut > 0),
+ * else HEGET_EINVAL; weight must not be NULL.
  *   momenta [dev] double[N][n+2][4], weight [dev] double[N]; both written. */
 int heget_gen_events(heget_ctx* ctx, uint64_t seed, int n, const heget_gen_cfg* cfg,
                      uint64_t first_event, int64_t N, double* momenta, double* weight,
@@ -98,10 +108,11 @@ int heget_gen_events(heget_ctx* ctx, uint64_t seed, int n, const heget_gen_cfg* 
  * PAPER.md:435-439), the fvixx0 chain through the propagators (p1 - K_l)/t_l of eqs. (7),(8)
  * over all n! photon orderings of eq. (6), walked
  * as a depth-first permutation tree with every prefix computed once, closed by iovxxx
- * (for n >= 4 the two orderings below a prefix of n-2 photons are closed
- * together through a per-event table built from the ubar side; for n >= 5 each fvixx0 of the
- * walk is evaluated in factorised form, a complex number times a per-(subset, photon) vector,
- * which the rank-one polarisation blocks of massless photons allow), squared and
+ * (the two orderings below a prefix of n-2 photons are closed together
+ * through a per-event table built from the ubar side; each fvixx0 of the walk is evaluated in
+ * factorised form, a complex number times a per-(subset, photon) vector, which the rank-one
+ * polarisation blocks of massless photons allow; n <= 4: one thread per event, n >= 5: one
+ * lane per photon-helicity assignment), squared and
  * summed over all 4*2^n helicities:
  *   out_amp2[e] = sum_{sigma1,sigma2,lambda_1..lambda_n} |M|^2   (the sum in eq. 2,
  *   PAPER.md:37, WITHOUT 1/(2 s_hat), spin/colour average and 1/n!).
@@ -121,7 +132,7 @@ int heget_amp2(heget_ctx* ctx, const double* momenta, int n, int precision, doub
  *                      Same result up to rounding order; NOT the permutation-tree method, hence a
  *                      separately named mode (reuse of off-shell lines).
  *   HEGET_ALGO_TREE2   two-sided chaining: the permutation tree from the u end (fvixx0) is walked
- *                      to depth n - min(n,3) only and every branch closes with one dot product
+ *                      to depth n - KS only, KS = min(n,4), and every branch closes with one dot product
  *                      against row vectors chained from the ubar end (fvoxx0 of List 2,
  *                      PAPER.md:449-450, 642-656) and tabulated per photon set: the same n!
  *                      diagrams with the off-shell lines near the ubar end shared.
@@ -141,22 +152,6 @@ int heget_amp2_algo(heget_ctx* ctx, const double* momenta, int n, int precision,
 int heget_amp2_sampled(heget_ctx* ctx, uint64_t seed, uint64_t first_event, const double* momenta,
                        int n, int precision, double* out_amp2, int32_t* out_hel, int64_t N,
                        void* stream);
-
-/* The paper's own program, List 2 generalised to n photons, run the way the
- * paper runs it: one thread per event, one drawn helicity assignment per event, 4-component HEGET
- * functions on cmplx w[6] (ixxxx1, oxxxx2, vxxxx0, n-1 fvoxx0 chained from the ubar line and one
- * iovxxx per permutation, iPNext through the n! orderings), no prefix reuse, no tables.  Same
- * arguments, helicity draw and result as heget_amp2_sampled (4 * 2^n * |M(h_e)|^2): it is the
- * design this library is measured against on the same GPU. */
-int heget_list2(heget_ctx* ctx, uint64_t seed, uint64_t first_event, const double* momenta, int n,
-                int precision, double* out_amp2, int32_t* out_hel, int64_t N, void* stream);
-
-/* The same program called for every one of the 4 * 2^n helicity assignments inside the thread:
- * out_amp2[e] = sum |M|^2, the quantity heget_amp2 returns, computed with the paper's arithmetic
- * (no prefix reuse, no parity, 4-component; SURVEY 8(d) model A).  A same-GPU baseline for the
- * headline metric; n = 7, 8 take minutes per 10^4 events. */
-int heget_list2_sum(heget_ctx* ctx, const double* momenta, int n, int precision, double* out_amp2,
-                    int64_t N, void* stream);
 
 /* Kinematical distributions of Fig. 2 as weighted histograms, filled on the
  * device: event e adds value[e] (e.g. weight * amp2; 0 = event failed the cuts, skipped) at
@@ -204,6 +199,8 @@ int heget_helas_vertex(heget_ctx* ctx, int fn, int precision, const double* fi, 
  * (helicity average, colour factor and identical-photon factor of eq. 2, PAPER.md:37;
  * DESIGN.md R1 for the colour factor),
  *   out3 = { sum_e x_e, sum_e x_e^2, #(weight[e] != 0) }   accumulated in fp64.
+ * An event with weight[e] == 0 (failed the cuts) contributes exactly 0 whatever amp2[e] holds, NaN
+ * and Inf included (R26: such events are what the cuts remove).
  * The result is deterministic (fixed reduction tree, no floating-point atomics).
  *   amp2, weight [dev] const double[N]; out3 [dev] double[3], written. */
 int heget_xsec_reduce(heget_ctx* ctx, const double* amp2, const double* weight, int n, int64_t N,
@@ -216,24 +213,6 @@ int heget_xsec_reduce(heget_ctx* ctx, const double* amp2, const double* weight, 
  *   out_amp2 [host] double[N] or NULL; out3 [host] double[3]. */
 int heget_xsec_host(heget_ctx* ctx, const double* momenta, const double* weight, int n,
                     int precision, int64_t N, double* out_amp2, double* out3);
-
-/* Peak-rate microbenchmark used for the roofline denominator: launches a kernel of
- * independent FMA chains (precision = HEGET_FP32 / HEGET_FP64) filling every SM and
- * writes the achieved FLOP/s (FMA = 2) to *flops_per_s [host].  Synchronises. */
-int heget_fma_peak(heget_ctx* ctx, int precision, double* flops_per_s);
-
-/* The same measurement for other operand patterns (context for the roofline: the amplitude
- * kernels' FMAs take three register operands, which the register file cannot feed at the
- * pipe's peak rate):
- *   HEGET_PEAK_CONST_OPERAND  x = x*a + b, a and b constant-bank operands (= heget_fma_peak)
- *   HEGET_PEAK_THREE_REG      x = y*z + x, three distinct registers, no operand reuse
- *   HEGET_PEAK_NODE_PATTERN   the fvixx0 node (16 FMA + 4 MUL per node, 36 flop) on registers */
-enum { HEGET_PEAK_CONST_OPERAND = 0, HEGET_PEAK_THREE_REG = 1, HEGET_PEAK_NODE_PATTERN = 2 };
-int heget_fma_peak_pattern(heget_ctx* ctx, int precision, int pattern, double* flops_per_s);
-
-/* Number of kernel launches this context has issued (all entry points), for bench.py's
- * gpu_launches count. */
-int64_t heget_launch_count(const heget_ctx* ctx);
 
 #ifdef __cplusplus
 }

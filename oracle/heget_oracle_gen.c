@@ -212,10 +212,13 @@ void heget_oracle_xsec_reduce(const double *amp2, const double *weight, int64_t 
     long double s1 = 0, s2 = 0;
     int64_t cnt = 0;
     for (int64_t e = 0; e < N; ++e) {
+        /* weight 0 = the event failed the cuts of eq. (9) and is not part of the
+         * integral: it contributes 0 whatever amp2 holds (reading R26) */
+        if (weight[e] == 0.0) continue;
         const long double x = (long double)weight[e] * (long double)amp2[e] * cf;
         s1 += x;
         s2 += x * x;
-        if (weight[e] != 0.0) ++cnt;
+        ++cnt;
     }
     out3[0] = (double)s1;
     out3[1] = (double)s2;

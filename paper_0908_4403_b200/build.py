@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 BUILD = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libheget.so")
-SOURCES = ["api.cu", "amp2.cu", "amp2_subset.cu", "amp2_twosided.cu", "amp2_sampled.cu", "hist.cu", "helas_eval.cu", "paper_program.cu", "gen.cu", "reduce.cu", "fma_peak.cu"]
+SOURCES = ["api.cu", "amp2.cu", "amp2_thread.cu", "amp2_subset.cu", "amp2_twosided.cu", "amp2_sampled.cu", "hist.cu", "helas_eval.cu", "paper_program.cu", "gen.cu", "reduce.cu", "fma_peak.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
@@ -26,6 +26,7 @@ def _nvcc():
 def _deps():
     out = [os.path.join(CSRC, f) for f in os.listdir(CSRC)]
     out.append(os.path.join(os.path.dirname(HERE), "include", "heget.h"))
+    out.append(os.path.join(os.path.dirname(HERE), "include", "heget_bench.h"))
     return out
 
 

@@ -53,6 +53,12 @@
 template <int N>
 using TreeGeometry = Geometry<N, HEGET_TREE_CTA_THREADS>;
 
+// n <= HEGET_THREAD_MAXN runs one thread per event (amp2_thread.cu); the lane-per-helicity kernel below
+// serves the larger n
+#ifndef HEGET_THREAD_MAXN
+#define HEGET_THREAD_MAXN 4
+#endif
+
 namespace {
 
 #ifndef HEGET_SHARE32_MAXN
@@ -280,6 +286,7 @@ cudaError_t heget_launch_amp2(const heget_ctx* ctx, const double* momenta, int n
 {
     *launches = 0;
     if (N == 0) return cudaSuccess;
+    if (n <= HEGET_THREAD_MAXN) return heget_launch_amp2_thread(ctx, momenta, n, precision, out_amp2, N, stream, launches);
     *launches = 1;
     if (precision == HEGET_FP32) return launch_n<float>(ctx, n, momenta, out_amp2, N, ctx->g, stream);
     return launch_n<double>(ctx, n, momenta, out_amp2, N, ctx->g, stream);

@@ -1,0 +1,433 @@
+// amp2_thread.cu -- heget_amp2 for n = 2, 3, 4: one THREAD per event (product code).
+//
+// This is the paper's own mapping (one phase-space point per thread) applied to the
+// permutation tree of eq. (6) in the two-component, factorised form of amp2_tables.cuh
+// and amp2_chain.cuh.  For n <= 4 an event's whole tree, for ALL 2^n photon-helicity assignments, fits
+// one thread's registers (2^n complex accumulators) plus a few per-thread columns of shared memory,
+// and the thread never idles: the lane-per-helicity kernel of amp2.cu spends most of a 4-photon event
+// in table phases that occupy 4, 6 or 14 of an event's 16 lanes and in the index arithmetic of its
+// work-item loops, which here is all folded at compile time.
+//
+// Per event (sigma_1 = +1 only; parity doubles it, sigma_1 = sigma_2 vanishes):
+//   a1  the thread reads its event's (n+2) four-vectors with 16-byte loads;
+//   a4  vxxxx0 of every photon, both helicities: E' entries (a, b) (make_photon_entries);
+//   a5  every non-empty proper subset S: P_S = -g/t_S (p1 - K_S)-slash block.  The components are
+//       light-cone sums in plain fp64; t_S of eq. (8) is exact on the fp64 inputs as
+//       given (reading R10) from per-event invariants held as unevaluated double-double sums,
+//           t_S = sum_{i in S} (k_i.k_i - 2 p1.k_i) + sum_{i<j in S} 2 k_i.k_j ,
+//       n(n+3)/2 Minkowski products per event instead of a double-double four-vector per subset
+//       (the fp32 kernel takes t_S = p+ p- - pT^2 in plain fp64);
+//   a6  fvixx0 nodes in factorised form psi = z v: v(S, i, h_i) = P_S (-1, a_i)^T, rho = v_0 + b_j v_1;
+//       every ordered prefix of up to n-2 photons is one node, computed once per helicity
+//       assignment OF THE PREFIX (2^|S| values, not 2^n);
+//   a7  the two orderings below a prefix of n-2 photons close with the pair closing row
+//       W_ab = U_b E'_a + U_a E'_b (U_b = <vbar| E'_b P_{all\b}); with the rank-one form of E',
+//       row . E' = (-u_0 + a u_1) (1, b).  For n = 4 the two ordered prefixes (i,j), (j,i) of a pair close
+//       with the same rows: ampsum(h) += W_ab(h_a,h_b) . [psi_2(i,j) + psi_2(j,i)](h_i,h_j);
+//   a8  sum_h |ampsum(h)|^2 and the constant factors, one 8-byte store.
+// Shared memory (n = 4 only): the thread's 8 vectors v({i}, i, h), 8 closing rows U_b(h) and 6 pair
+// entries P_{ij}, as columns [word][thread] (conflict-free 16-byte / 8-byte accesses).
+#include "amp2_chain.cuh"
+
+namespace {
+
+#ifndef HEGET_THREAD_CTA
+#define HEGET_THREAD_CTA 64        // threads (= events) per CTA
+#endif
+#ifndef HEGET_THREAD_MINB64_N4
+#define HEGET_THREAD_MINB64_N4 4   // __launch_bounds__ min CTAs per SM: fp64 4 photons (255 registers)
+#endif
+#ifndef HEGET_THREAD_MINB32_N4
+#define HEGET_THREAD_MINB32_N4 6
+#endif
+#ifndef HEGET_THREAD_MINB_SMALL
+#define HEGET_THREAD_MINB_SMALL 6  // n = 2, 3
+#endif
+
+// unevaluated sum hi + lo; not normalised (lo may be comparable to hi after cancellation)
+__device__ __forceinline__ void dd_add_to(dd& a, const dd& b)
+{
+    const dd s = dd_two_sum(a.hi, b.hi);
+    a.hi = s.hi;
+    a.lo = __dadd_rn(a.lo, __dadd_rn(s.lo, b.lo));
+}
+
+// a.b = a0 b0 - a1 b1 - a2 b2 - a3 b3 as an unevaluated sum: exact products (FMA), the high parts
+// summed by TwoSum, every rounding error collected in lo
+__device__ __forceinline__ dd dd_minkowski(const double (&a)[4], const double (&b)[4])
+{
+    const dd p0 = dd_two_prod(a[0], b[0]), p1 = dd_two_prod(a[1], b[1]), p2 = dd_two_prod(a[2], b[2]),
+             p3 = dd_two_prod(a[3], b[3]);
+    const dd s1 = dd_two_sum(p0.hi, -p1.hi), s2 = dd_two_sum(s1.hi, -p2.hi), s3 = dd_two_sum(s2.hi, -p3.hi);
+    const double lo = __dadd_rn(__dadd_rn(__dsub_rn(__dsub_rn(__dsub_rn(p0.lo, p1.lo), p2.lo), p3.lo), s1.lo),
+                                __dadd_rn(s2.lo, s3.lo));
+    return {s3.hi, lo};
+}
+
+template <typename T>
+__device__ __forceinline__ Cx<T> cx_mul(const Cx<T>& a, const Cx<T>& b)
+{
+    return {fma(a.r, b.r, -(a.i * b.i)), fma(a.r, b.i, a.i * b.r)};
+}
+
+// -u_0 + a u_1 for a row u = (u_0, u_1): the scalar of row . E' = (-u_0 + a u_1) (1, b)
+template <typename T>
+__device__ __forceinline__ Cx<T> row_scalar(const Spinor<T>& u, const EEntry<T>& e)
+{
+    return {fma(e.ar, u.r1, fma(-e.ai, u.i1, -u.r0)), fma(e.ar, u.i1, fma(e.ai, u.r1, -u.i0))};
+}
+
+// W . v (two-component dot product, no conjugation)
+template <typename T>
+__device__ __forceinline__ Cx<T> row_dot(const Spinor<T>& w, const Spinor<T>& v)
+{
+    return {fma(w.r0, v.r0, fma(-w.i0, v.i0, fma(w.r1, v.r1, -(w.i1 * v.i1)))),
+            fma(w.r0, v.i0, fma(w.i0, v.r0, fma(w.r1, v.i1, w.i1 * v.r1)))};
+}
+
+// Per-event kinematics shared by all subsets: light-cone components of every photon and, for the
+// fp64 kernel, the invariants c_i = k_i.k_i - 2 p1.k_i and d_ij = 2 k_i.k_j as double-doubles.
+template <int N, bool EXACT>
+struct Kinematics {
+    double kp[N], km[N], kx[N], ky[N];
+    double two_e1, coupling;   // 2 E1; -g * scale
+    dd c[EXACT ? N : 1];
+    dd d[EXACT ? N * (N - 1) / 2 : 1];   // pair i < j at j (j - 1) / 2 + i
+
+    __device__ __forceinline__ void init(const double (&k)[N][4], double e1, double g, double scale)
+    {
+        two_e1 = 2.0 * e1;
+        coupling = -g * scale;
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+            kp[i] = k[i][0] + k[i][3];
+            km[i] = k[i][0] - k[i][3];
+            kx[i] = k[i][1];
+            ky[i] = k[i][2];
+        }
+        if constexpr (EXACT) {
+#pragma unroll
+            for (int i = 0; i < N; ++i) {
+                // p1 = (E1, 0, 0, E1): 2 p1.k_i = 2 E1 (w_i - kz_i), the difference by TwoSum
+                const dd u = dd_two_sum(k[i][0], -k[i][3]);
+                dd q = dd_two_prod(two_e1, u.hi);
+                q.lo = __fma_rn(two_e1, u.lo, q.lo);
+                c[i] = dd_minkowski(k[i], k[i]);
+                dd_add_to(c[i], dd_neg(q));
+            }
+#pragma unroll
+            for (int j = 1; j < N; ++j)
+#pragma unroll
+                for (int i = 0; i < j; ++i) {
+                    const dd m = dd_minkowski(k[i], k[j]);
+                    d[j * (j - 1) / 2 + i] = {2.0 * m.hi, 2.0 * m.lo};
+                }
+        }
+    }
+
+    // P entry of subset S (compile-time constant after unrolling)
+    template <typename T>
+    __device__ __forceinline__ PEntry<T> subset(unsigned S) const
+    {
+        double skp = 0.0, skm = 0.0, skx = 0.0, sky = 0.0;
+#pragma unroll
+        for (int i = 0; i < N; ++i)
+            if ((S >> i) & 1u) {
+                skp += kp[i];
+                skm += km[i];
+                skx += kx[i];
+                sky += ky[i];
+            }
+        const double pp = two_e1 - skp;
+        double t;
+        if constexpr (EXACT) {
+            dd acc = {0.0, 0.0};
+            bool first = true;
+#pragma unroll
+            for (int i = 0; i < N; ++i)
+                if ((S >> i) & 1u) {
+                    if (first) acc = c[i]; else dd_add_to(acc, c[i]);
+                    first = false;
+                }
+#pragma unroll
+            for (int j = 1; j < N; ++j)
+#pragma unroll
+                for (int i = 0; i < j; ++i)
+                    if (((S >> i) & 1u) && ((S >> j) & 1u)) dd_add_to(acc, d[j * (j - 1) / 2 + i]);
+            t = __dadd_rn(acc.hi, acc.lo);
+        } else {
+            t = -fma(pp, skm, fma(skx, skx, sky * sky));   // p+ p- - pT^2, both terms <= 0
+        }
+        const double f = coupling * fast_rcp(t);
+        PEntry<T> out;
+        out.pp = (T)(f * pp);
+        out.pm = (T)(-f * skm);
+        out.px = (T)(-f * skx);
+        out.py = (T)(-f * sky);
+        return out;
+    }
+};
+
+// per-thread column store in shared memory: word w of this thread at col[w * CTA]
+template <typename T>
+__device__ __forceinline__ void put(Cx<T>* col, int w, const Spinor<T>& s)
+{
+    col[(2 * w) * HEGET_THREAD_CTA] = {s.r0, s.i0};
+    col[(2 * w + 1) * HEGET_THREAD_CTA] = {s.r1, s.i1};
+}
+template <typename T>
+__device__ __forceinline__ Spinor<T> get(const Cx<T>* col, int w)
+{
+    const Cx<T> a = col[(2 * w) * HEGET_THREAD_CTA], b = col[(2 * w + 1) * HEGET_THREAD_CTA];
+    return {a.r, a.i, b.r, b.i};
+}
+template <typename T>
+__device__ __forceinline__ void put(Cx<T>* col, int w, const PEntry<T>& p)
+{
+    col[(2 * w) * HEGET_THREAD_CTA] = {p.pp, p.pm};
+    col[(2 * w + 1) * HEGET_THREAD_CTA] = {p.px, p.py};
+}
+template <typename T>
+__device__ __forceinline__ PEntry<T> get_p(const Cx<T>* col, int w)
+{
+    const Cx<T> a = col[(2 * w) * HEGET_THREAD_CTA], b = col[(2 * w + 1) * HEGET_THREAD_CTA];
+    return {a.r, a.i, b.r, b.i};
+}
+
+// pair closing row W_ab(h_a, h_b) = U_b(h_b) E'_a(h_a) + U_a(h_a) E'_b(h_b), rank-one form of E'
+template <typename T>
+__device__ __forceinline__ Spinor<T> pair_row(const Spinor<T>& ua, const Spinor<T>& ub, const EEntry<T>& ea,
+                                              const EEntry<T>& eb)
+{
+    const Cx<T> sba = row_scalar(ub, ea), sab = row_scalar(ua, eb);
+    const Cx<T> ba = {ea.br, ea.bi}, bb = {eb.br, eb.bi};
+    const Cx<T> x = cx_mul(sba, ba);
+    Spinor<T> w;
+    w.r0 = sba.r + sab.r;
+    w.i0 = sba.i + sab.i;
+    w.r1 = fma(sab.r, bb.r, fma(-sab.i, bb.i, x.r));
+    w.i1 = fma(sab.r, bb.i, fma(sab.i, bb.r, x.i));
+    return w;
+}
+
+constexpr int kColumnWords4 = 2 * (8 + 8 + 6);   // Cx words per thread, n = 4: v1[8], U[8], P_ij[6]
+
+template <int N, typename T>
+constexpr int kMinBlocks = (N == 4) ? ((sizeof(T) == 8) ? HEGET_THREAD_MINB64_N4 : HEGET_THREAD_MINB32_N4)
+                                    : HEGET_THREAD_MINB_SMALL;
+
+template <int N, typename T>
+__global__ void __launch_bounds__(HEGET_THREAD_CTA, kMinBlocks<N, T>)
+amp2_thread_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_t n_events, double g)
+{
+    static_assert(N >= 2 && N <= 4, "one thread per event holds 2^N accumulators: n <= 4");
+    constexpr int L = 1 << N;
+    constexpr unsigned ALL = L - 1;
+    __shared__ Cx<T> s_col[(N == 4) ? kColumnWords4 * HEGET_THREAD_CTA : 1];
+
+    int64_t ev = (int64_t)blockIdx.x * HEGET_THREAD_CTA + threadIdx.x;
+    const bool live = ev < n_events;
+    if (!live) ev = n_events - 1;
+
+    // a1: (n+2) four-vectors, 16-byte loads
+    double e1, e2, k[N][4];
+    {
+        const double2* src = reinterpret_cast<const double2*>(momenta) + ev * (2 * (N + 2));
+        e1 = __ldg(src).x;
+        e2 = __ldg(src + 2).x;
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+            const double2 a = __ldg(src + 4 + 2 * i), b = __ldg(src + 5 + 2 * i);
+            k[i][0] = a.x; k[i][1] = a.y; k[i][2] = b.x; k[i][3] = b.y;
+        }
+    }
+    const double shat = 4.0 * e1 * e2;
+    const double scale = (sizeof(T) == 4) ? sqrt(shat) : 1.0;   // fp32 works in units of sqrt(s_hat)
+
+    // a4: E' entries e[i][h], h = 1: lambda = +1
+    EEntry<T> e[N][2];
+    double norm = 2.0 * g * g * shat;   // 2 (parity) g^2 (closing vertex) s_hat (spinor norms) prod s_i^2 / 2
+#pragma unroll
+    for (int i = 0; i < N; ++i) norm *= 0.5 * make_photon_entries<T>(k[i], &e[i][1], &e[i][0]);
+    if constexpr (sizeof(T) == 4) {
+        const double inv = 1.0 / shat;
+#pragma unroll
+        for (int i = 0; i < N - 1; ++i) norm *= inv;
+    }
+
+    // a5: kinematic invariants of the event
+    Kinematics<N, sizeof(T) == 8> kin;
+    kin.init(k, e1, g, scale);
+
+    Cx<T> amp[L];
+#pragma unroll
+    for (int h = 0; h < L; ++h) amp[h] = {(T)0, (T)0};
+
+    if constexpr (N == 2) {
+        // ampsum(h) = W_01(h_0, h_1) . (1, 0): the two diagrams
+        Spinor<T> u[2][2];
+#pragma unroll
+        for (int b = 0; b < 2; ++b) {
+            const PEntry<T> p = kin.template subset<T>(ALL ^ (1u << b));
+#pragma unroll
+            for (int h = 0; h < 2; ++h) u[b][h] = closing_entry(e[b][h], p);
+        }
+#pragma unroll
+        for (int h0 = 0; h0 < 2; ++h0)
+#pragma unroll
+            for (int h1 = 0; h1 < 2; ++h1) {
+                const Spinor<T> w = pair_row(u[0][h0], u[1][h1], e[0][h0], e[1][h1]);
+                amp[h0 | (h1 << 1)] = {w.r0, w.i0};
+            }
+    } else if constexpr (N == 3) {
+        Spinor<T> u[3][2];
+#pragma unroll
+        for (int b = 0; b < 3; ++b) {
+            const PEntry<T> p = kin.template subset<T>(ALL ^ (1u << b));
+#pragma unroll
+            for (int h = 0; h < 2; ++h) u[b][h] = closing_entry(e[b][h], p);
+        }
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+            const int a = (i == 0) ? 1 : 0, b = (i == 2) ? 1 : 2;   // the other two, a < b
+            const PEntry<T> p = kin.template subset<T>(1u << i);
+            Spinor<T> v[2];
+#pragma unroll
+            for (int h = 0; h < 2; ++h) v[h] = chain_vector(p, e[i][h]);
+#pragma unroll
+            for (int ha = 0; ha < 2; ++ha)
+#pragma unroll
+                for (int hb = 0; hb < 2; ++hb) {
+                    const Spinor<T> w = pair_row(u[a][ha], u[b][hb], e[a][ha], e[b][hb]);
+#pragma unroll
+                    for (int hi = 0; hi < 2; ++hi) {
+                        const Cx<T> kk = row_dot(w, v[hi]);
+                        const int h = (hi << i) | (ha << a) | (hb << b);
+                        amp[h].r += kk.r;
+                        amp[h].i += kk.i;
+                    }
+                }
+        }
+    } else {
+        Cx<T>* col = s_col + threadIdx.x;
+        // tables: v1[2 i + h] = v({i}, i, h), U[2 b + h], P_ij at pair index j (j - 1) / 2 + i
+        constexpr int V1 = 0, UU = 8, PP = 16;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const PEntry<T> p1 = kin.template subset<T>(1u << i);
+            const PEntry<T> p3 = kin.template subset<T>(ALL ^ (1u << i));
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                put(col, V1 + 2 * i + h, chain_vector(p1, e[i][h]));
+                put(col, UU + 2 * i + h, closing_entry(e[i][h], p3));
+            }
+        }
+#pragma unroll
+        for (int j = 1; j < 4; ++j)
+#pragma unroll
+            for (int i = 0; i < j; ++i)
+                put(col, PP + j * (j - 1) / 2 + i, kin.template subset<T>((1u << i) | (1u << j)));
+        // the columns are private to the thread; the fence only keeps the compiler from forwarding the
+        // stored values through registers (which spills) instead of reloading them where they are used
+        __syncwarp();
+
+        // the 12 ordered prefixes (i, j), grouped by the unordered pair: both close with W_ab, {a,b} the rest
+#pragma unroll
+        for (int j = 1; j < 4; ++j)
+#pragma unroll
+            for (int i = 0; i < j; ++i) {
+                const unsigned rest = ALL ^ (1u << i) ^ (1u << j);   // {a < b}: folded after unrolling
+                const int a = (rest & 1u) ? 0 : ((rest & 2u) ? 1 : 2);
+                const int b = (rest & 8u) ? 3 : ((rest & 4u) ? 2 : 1);
+                // Psi(h_i, h_j) = psi_2(i, j) + psi_2(j, i): the two ordered prefixes of {i, j}, each
+                // rho(f -> l) v({i,j}, l), close with the same rows W_ab (distributivity)
+                const PEntry<T> pij = get_p(col, PP + j * (j - 1) / 2 + i);
+                Spinor<T> psi[2][2];   // [h_i][h_j]
+                {
+                    Spinor<T> v2i[2], v2j[2];
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        v2i[h] = chain_vector(pij, e[i][h]);
+                        v2j[h] = chain_vector(pij, e[j][h]);
+                    }
+#pragma unroll
+                    for (int hi = 0; hi < 2; ++hi) {
+                        const Spinor<T> v1i = get(col, V1 + 2 * i + hi);
+#pragma unroll
+                        for (int hj = 0; hj < 2; ++hj) {
+                            Cx<T> r;
+                            chain_rho(v1i, e[j][hj], r.r, r.i);
+                            psi[hi][hj].r0 = fma(r.r, v2j[hj].r0, -(r.i * v2j[hj].i0));
+                            psi[hi][hj].i0 = fma(r.r, v2j[hj].i0, r.i * v2j[hj].r0);
+                            psi[hi][hj].r1 = fma(r.r, v2j[hj].r1, -(r.i * v2j[hj].i1));
+                            psi[hi][hj].i1 = fma(r.r, v2j[hj].i1, r.i * v2j[hj].r1);
+                        }
+                    }
+#pragma unroll
+                    for (int hj = 0; hj < 2; ++hj) {
+                        const Spinor<T> v1j = get(col, V1 + 2 * j + hj);
+#pragma unroll
+                        for (int hi = 0; hi < 2; ++hi) {
+                            Cx<T> r;
+                            chain_rho(v1j, e[i][hi], r.r, r.i);
+                            psi[hi][hj].r0 = fma(r.r, v2i[hi].r0, fma(-r.i, v2i[hi].i0, psi[hi][hj].r0));
+                            psi[hi][hj].i0 = fma(r.r, v2i[hi].i0, fma(r.i, v2i[hi].r0, psi[hi][hj].i0));
+                            psi[hi][hj].r1 = fma(r.r, v2i[hi].r1, fma(-r.i, v2i[hi].i1, psi[hi][hj].r1));
+                            psi[hi][hj].i1 = fma(r.r, v2i[hi].i1, fma(r.i, v2i[hi].r1, psi[hi][hj].i1));
+                        }
+                    }
+                }
+#pragma unroll
+                for (int ha = 0; ha < 2; ++ha) {
+                    const Spinor<T> ua = get(col, UU + 2 * a + ha);
+#pragma unroll
+                    for (int hb = 0; hb < 2; ++hb) {
+                        const Spinor<T> w = pair_row(ua, get(col, UU + 2 * b + hb), e[a][ha], e[b][hb]);
+#pragma unroll
+                        for (int hi = 0; hi < 2; ++hi)
+#pragma unroll
+                            for (int hj = 0; hj < 2; ++hj) {
+                                const int h = (hi << i) | (hj << j) | (ha << a) | (hb << b);
+                                const Cx<T> kk = row_dot(w, psi[hi][hj]);
+                                amp[h].r += kk.r;
+                                amp[h].i += kk.i;
+                            }
+                    }
+                }
+            }
+    }
+
+    // a8
+    double m2 = 0.0;
+#pragma unroll
+    for (int h = 0; h < L; ++h) m2 += (double)amp[h].r * (double)amp[h].r + (double)amp[h].i * (double)amp[h].i;
+    if (live) out[ev] = norm * m2;
+}
+
+template <int N, typename T>
+cudaError_t launch_thread(const double* momenta, double* out, int64_t n_events, double g, cudaStream_t stream)
+{
+    const int64_t blocks = (n_events + HEGET_THREAD_CTA - 1) / HEGET_THREAD_CTA;
+    amp2_thread_kernel<N, T><<<(unsigned)blocks, HEGET_THREAD_CTA, 0, stream>>>(momenta, out, n_events, g);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+cudaError_t heget_launch_amp2_thread(const heget_ctx* ctx, const double* momenta, int n, int precision,
+                                     double* out_amp2, int64_t N, cudaStream_t stream, int* launches)
+{
+    *launches = 0;
+    if (N == 0) return cudaSuccess;
+    *launches = 1;
+    const bool f32 = precision == HEGET_FP32;
+    switch (n) {
+        case 2: return f32 ? launch_thread<2, float>(momenta, out_amp2, N, ctx->g, stream)
+                           : launch_thread<2, double>(momenta, out_amp2, N, ctx->g, stream);
+        case 3: return f32 ? launch_thread<3, float>(momenta, out_amp2, N, ctx->g, stream)
+                           : launch_thread<3, double>(momenta, out_amp2, N, ctx->g, stream);
+        case 4: return f32 ? launch_thread<4, float>(momenta, out_amp2, N, ctx->g, stream)
+                           : launch_thread<4, double>(momenta, out_amp2, N, ctx->g, stream);
+        default: return cudaErrorInvalidValue;
+    }
+}

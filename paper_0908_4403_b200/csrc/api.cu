@@ -40,12 +40,36 @@ void free_staging(heget_ctx* ctx)
 
 }  // namespace
 
+namespace {
+int gen_events(heget_ctx* ctx, uint64_t seed, int n, const heget_gen_cfg* cfg, uint64_t first_event, int64_t N,
+               double* momenta, double* weight, void* stream)
+{
+    if (!ctx || !cfg || n < 2 || n > 8 || N < 0 || N > HEGET_MAX_EVENTS || (N > 0 && !momenta)) return HEGET_EINVAL;
+    if (cfg->mode < HEGET_GEN_FIXED || cfg->mode > HEGET_GEN_TOYPDF || !(cfg->a > 0.0) || !std::isfinite(cfg->a)) return HEGET_EINVAL;
+    if (cfg->mode == HEGET_GEN_LOGUNIFORM && (!(cfg->b >= cfg->a) || !std::isfinite(cfg->b) || !std::isfinite(cfg->y_max))) return HEGET_EINVAL;
+    if (cfg->mode == HEGET_GEN_TOYPDF) {
+        // tau = x1 x2 is drawn log-uniform in [tau_min, 1], tau_min = (n pt_cut)^2 / s (R19)
+        const double tau_min = (n * ctx->pt_cut) * (n * ctx->pt_cut) / (cfg->a * cfg->a);
+        if (!(tau_min > 0.0) || !(tau_min < 1.0)) return HEGET_EINVAL;
+    }
+    DeviceGuard guard(ctx->device);
+    if (!guard.ok) return fail_cuda(ctx, cudaGetLastError());
+    int launches = 0;
+    cudaError_t err = heget_launch_gen(ctx, seed, n, cfg, first_event, N, momenta, weight, (cudaStream_t)stream, &launches);
+    ctx->launches += launches;
+    return err == cudaSuccess ? HEGET_OK : fail_cuda(ctx, err);
+}
+}  // namespace
+
 extern "C" {
 
 int heget_init(int device, double alpha, double q_charge, double pt_cut, double eta_cut, double dr_cut,
                heget_ctx** out)
 {
     if (!out || !(alpha > 0.0) || device < 0) return HEGET_EINVAL;
+    if (!std::isfinite(alpha) || !std::isfinite(q_charge) || !std::isfinite(pt_cut) || !std::isfinite(eta_cut) ||
+        !std::isfinite(dr_cut) || pt_cut < 0.0 || eta_cut < 0.0 || dr_cut < 0.0)
+        return HEGET_EINVAL;
     int count = 0;
     if (cudaGetDeviceCount(&count) != cudaSuccess || device >= count) return HEGET_ECUDA;
     DeviceGuard guard(device);
@@ -64,7 +88,7 @@ int heget_init(int device, double alpha, double q_charge, double pt_cut, double 
     cudaError_t err = cudaGetDeviceProperties(&prop, device);
     if (err == cudaSuccess) {
         ctx->sm_count = prop.multiProcessorCount;
-        err = cudaMalloc(&ctx->d_partials, sizeof(double) * 3 * kReduceBlocks);
+        err = cudaMalloc(&ctx->d_partials, sizeof(double) * 3 * kReduceBlocks * (HEGET_REDUCE_SLOTS + 1));
     }
     if (err == cudaSuccess) err = cudaMalloc(&ctx->d_stage_out3, sizeof(double) * 3);
     if (err == cudaSuccess) err = cudaStreamCreateWithFlags(&ctx->host_stream, cudaStreamNonBlocking);
@@ -117,15 +141,9 @@ int64_t heget_launch_count(const heget_ctx* ctx) { return ctx ? ctx->launches : 
 int heget_gen_events(heget_ctx* ctx, uint64_t seed, int n, const heget_gen_cfg* cfg, uint64_t first_event,
                      int64_t N, double* momenta, double* weight, void* stream)
 {
-    if (!ctx || !cfg || n < 2 || n > 8 || N < 0 || N > HEGET_MAX_EVENTS || (N > 0 && !momenta)) return HEGET_EINVAL;
-    if (cfg->mode < HEGET_GEN_FIXED || cfg->mode > HEGET_GEN_TOYPDF || !(cfg->a > 0.0)) return HEGET_EINVAL;
-    if (cfg->mode == HEGET_GEN_LOGUNIFORM && !(cfg->b >= cfg->a)) return HEGET_EINVAL;
-    DeviceGuard guard(ctx->device);
-    if (!guard.ok) return fail_cuda(ctx, cudaGetLastError());
-    int launches = 0;
-    cudaError_t err = heget_launch_gen(ctx, seed, n, cfg, first_event, N, momenta, weight, (cudaStream_t)stream, &launches);
-    ctx->launches += launches;
-    return err == cudaSuccess ? HEGET_OK : fail_cuda(ctx, err);
+    if (N > 0 && !weight) return HEGET_EINVAL;   // only heget_rambo runs without a weight buffer
+    if ((reinterpret_cast<uintptr_t>(momenta) & 15u) != 0) return HEGET_EINVAL;
+    return gen_events(ctx, seed, n, cfg, first_event, N, momenta, weight, stream);
 }
 
 int heget_rambo(heget_ctx* ctx, uint64_t seed, int n, double sqrt_s_hat, int64_t N, double* momenta, void* stream)
@@ -136,7 +154,8 @@ int heget_rambo(heget_ctx* ctx, uint64_t seed, int n, double sqrt_s_hat, int64_t
     cfg.a = sqrt_s_hat;
     cfg.b = 0.0;
     cfg.y_max = 0.0;
-    return heget_gen_events(ctx, seed, n, &cfg, 0, N, momenta, nullptr, stream);
+    if ((reinterpret_cast<uintptr_t>(momenta) & 15u) != 0) return HEGET_EINVAL;
+    return gen_events(ctx, seed, n, &cfg, 0, N, momenta, nullptr, stream);
 }
 
 int heget_amp2(heget_ctx* ctx, const double* momenta, int n, int precision, double* out_amp2, int64_t N, void* stream)
@@ -266,7 +285,8 @@ int heget_xsec_reduce(heget_ctx* ctx, const double* amp2, const double* weight, 
     DeviceGuard guard(ctx->device);
     if (!guard.ok) return fail_cuda(ctx, cudaGetLastError());
     int launches = 0;
-    cudaError_t err = heget_launch_reduce(ctx, amp2, weight, n, N, out3, (cudaStream_t)stream, &launches);
+    double* partials = ctx->d_partials + (size_t)(ctx->reduce_slot++ % HEGET_REDUCE_SLOTS) * 3 * kReduceBlocks;
+    cudaError_t err = heget_launch_reduce(partials, amp2, weight, n, N, out3, (cudaStream_t)stream, &launches);
     ctx->launches += launches;
     return err == cudaSuccess ? HEGET_OK : fail_cuda(ctx, err);
 }
@@ -317,7 +337,9 @@ int heget_xsec_host(heget_ctx* ctx, const double* momenta, const double* weight,
             launches += l1;
         }
     }
-    if (err == cudaSuccess) err = heget_launch_reduce(ctx, ctx->d_stage_amp2, ctx->d_stage_w, n, N, ctx->d_stage_out3, st, &l2);
+    if (err == cudaSuccess)
+        err = heget_launch_reduce(ctx->d_partials + (size_t)HEGET_REDUCE_SLOTS * 3 * kReduceBlocks, ctx->d_stage_amp2,
+                                  ctx->d_stage_w, n, N, ctx->d_stage_out3, st, &l2);
     ctx->launches += launches + l2;
     if (err == cudaSuccess && out_amp2 && N > 0)
         err = cudaMemcpyAsync(out_amp2, ctx->d_stage_amp2, sizeof(double) * N, cudaMemcpyDeviceToHost, st);

@@ -26,13 +26,24 @@ __device__ __forceinline__ double phase_space_volume(int n, double s)
     return v;
 }
 
+constexpr int kGenThreads = 128;
+
+// One thread per event computes; the CTA's momenta go through shared memory (row stride padded by one
+// 16-byte word: conflict-free stores) and leave as ONE contiguous span of double2 words, the mirror of
+// MomentaTile::load in amp2_common.cuh (a thread writing its own (n+2) x 32 bytes at a stride of
+// 32 (n+2) bytes reached 20 % of the HBM write rate).
 template <int N>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(kGenThreads)
 gen_kernel(uint64_t seed, heget_gen_cfg cfg, double pt_cut, double eta_cut, double dr_cut,
            uint64_t first_event, int64_t n_events, double* __restrict__ momenta, double* __restrict__ weight)
 {
-    const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= n_events) return;
+    constexpr int WORDS = 2 * (N + 2);             // double2 words per event
+    constexpr int STRIDE = WORDS + 1;
+    __shared__ double2 s_out[kGenThreads * STRIDE];
+    const int64_t ev0 = (int64_t)blockIdx.x * kGenThreads;
+    int64_t e = ev0 + threadIdx.x;
+    const bool live = e < n_events;
+    if (!live) e = n_events - 1;                   // past the end: recompute the last event, store nothing
     const uint64_t ev = first_event + (uint64_t)e;
     const double pi = 3.14159265358979323846;
 
@@ -79,12 +90,12 @@ gen_kernel(uint64_t seed, heget_gen_cfg cfg, double pt_cut, double eta_cut, doub
     const double gam = Q[0] / M, a = 1.0 / (1.0 + gam), x = rs / M;
     const double ch = cosh(y), sh = sinh(y);
 
-    double* out = momenta + e * 4 * (N + 2);
+    double2* out = s_out + threadIdx.x * STRIDE;
     const double e1 = 0.5 * rs * exp(y), e2 = 0.5 * rs * exp(-y);
-    reinterpret_cast<double2*>(out)[0] = make_double2(e1, 0.0);
-    reinterpret_cast<double2*>(out)[1] = make_double2(0.0, e1);
-    reinterpret_cast<double2*>(out)[2] = make_double2(e2, 0.0);
-    reinterpret_cast<double2*>(out)[3] = make_double2(0.0, -e2);
+    out[0] = make_double2(e1, 0.0);
+    out[1] = make_double2(0.0, e1);
+    out[2] = make_double2(e2, 0.0);
+    out[3] = make_double2(0.0, -e2);
 
     bool pass = true;
     double eta[N], phi[N];
@@ -97,8 +108,8 @@ gen_kernel(uint64_t seed, heget_gen_cfg cfg, double pt_cut, double eta_cut, doub
         const double kz = x * (q[i][3] + b[2] * q[i][0] + a * bq * b[2]);
         const double E = k0 * ch + kz * sh;   // boost by y along z
         const double pz = kz * ch + k0 * sh;
-        reinterpret_cast<double2*>(out)[4 + 2 * i] = make_double2(E, kx);
-        reinterpret_cast<double2*>(out)[5 + 2 * i] = make_double2(ky, pz);
+        out[4 + 2 * i] = make_double2(E, kx);
+        out[5 + 2 * i] = make_double2(ky, pz);
         if (cfg.apply_cuts) {
             const double pt = sqrt(kx * kx + ky * ky);
             eta[i] = asinh(pz / pt);
@@ -117,17 +128,22 @@ gen_kernel(uint64_t seed, heget_gen_cfg cfg, double pt_cut, double eta_cut, doub
                 pass = pass && (sqrt(deta * deta + dphi * dphi) > dr_cut);
             }
     }
-    if (weight) {
+    if (weight && live) {
         const double shat = rs * rs;
         weight[e] = pass ? phase_space_volume(N, shat) / (2.0 * shat) * extra : 0.0;
     }
+    __syncthreads();
+    const int64_t left = n_events - ev0;
+    const int span = (int)(left < kGenThreads ? left : kGenThreads) * WORDS;
+    double2* dst = reinterpret_cast<double2*>(momenta) + ev0 * WORDS;
+    for (int idx = threadIdx.x; idx < span; idx += kGenThreads) dst[idx] = s_out[(idx / WORDS) * STRIDE + idx % WORDS];
 }
 
 template <int N>
 cudaError_t launch(const heget_ctx* ctx, uint64_t seed, const heget_gen_cfg& cfg, uint64_t first_event,
                    int64_t n_events, double* momenta, double* weight, cudaStream_t stream)
 {
-    const int threads = 128;
+    const int threads = kGenThreads;
     const int64_t blocks = (n_events + threads - 1) / threads;
     gen_kernel<N><<<(unsigned)blocks, threads, 0, stream>>>(seed, cfg, ctx->pt_cut, ctx->eta_cut, ctx->dr_cut,
                                                            first_event, n_events, momenta, weight);

@@ -5,6 +5,7 @@
 #include <stdint.h>
 
 #include "../../include/heget.h"
+#include "../../include/heget_bench.h"
 
 constexpr int kHostChunks = 8;  // pipeline depth of heget_xsec_host
 
@@ -15,7 +16,10 @@ struct heget_ctx {
     double g;  // gal[0] = gal[1] = -e Q_q (eq. 26)
     double pt_cut, eta_cut, dr_cut;
     // scratch owned by the context
-    double* d_partials;     // [kReduceBlocks][3] block partial sums of heget_xsec_reduce
+    double* d_partials;     // [HEGET_REDUCE_SLOTS + 1][kReduceBlocks][3] block partial sums of heget_xsec_reduce:
+                            // a ring used round-robin by the [dev] calls (they may run concurrently on
+                            // different streams), the last slot is heget_xsec_host's own
+    unsigned reduce_slot;   // next ring slot
     double* d_stage_mom;    // staging for the *_host entry point
     double* d_stage_w;
     double* d_stage_amp2;
@@ -34,6 +38,8 @@ constexpr int kReduceBlocks = 296;  // 2 CTAs per SM on a 148-SM B200; any value
 // launchers (each returns a cudaError_t from the launch)
 cudaError_t heget_launch_amp2(const heget_ctx* ctx, const double* momenta, int n, int precision,
                               double* out_amp2, int64_t N, cudaStream_t stream, int* launches);
+cudaError_t heget_launch_amp2_thread(const heget_ctx* ctx, const double* momenta, int n, int precision,
+                                     double* out_amp2, int64_t N, cudaStream_t stream, int* launches);
 cudaError_t heget_launch_amp2_subset(const heget_ctx* ctx, const double* momenta, int n, int precision,
                                      double* out_amp2, int64_t N, cudaStream_t stream, int* launches);
 cudaError_t heget_launch_amp2_twosided(const heget_ctx* ctx, const double* momenta, int n, int precision,
@@ -54,6 +60,6 @@ cudaError_t heget_launch_helas_vertex(int fn, int precision, const double* a, co
 cudaError_t heget_launch_gen(const heget_ctx* ctx, uint64_t seed, int n, const heget_gen_cfg* cfg,
                              uint64_t first_event, int64_t N, double* momenta, double* weight,
                              cudaStream_t stream, int* launches);
-cudaError_t heget_launch_reduce(const heget_ctx* ctx, const double* amp2, const double* weight, int n,
-                                int64_t N, double* out3, cudaStream_t stream, int* launches);
+cudaError_t heget_launch_reduce(double* partials /* [kReduceBlocks][3] */, const double* amp2, const double* weight,
+                                int n, int64_t N, double* out3, cudaStream_t stream, int* launches);
 cudaError_t heget_run_fma_peak(const heget_ctx* ctx, int precision, int pattern, double* flops_per_s, int* launches);

@@ -1,6 +1,6 @@
 // reduce.cu -- heget_xsec_reduce: step 6 of PAPER.md:141 on the device (product code).
-// x_e = weight[e] * amp2[e] * (1/4)(1/9)(1/n!)  (eq. 2); out3 = {sum x, sum x^2,
-// #(weight != 0)}.  Fixed reduction tree (grid-stride partials, warp shuffles, one final CTA):
+// x_e = weight[e] * amp2[e] * (1/4)(1/9)(1/n!)  (eq. 2; 0 where weight[e] == 0);
+// out3 = {sum x, sum x^2, #(weight != 0)}.  Fixed reduction tree (grid-stride partials, warp shuffles, one final CTA):
 // bit-reproducible from run to run, no floating-point atomics.
 #include "heget_internal.cuh"
 
@@ -43,7 +43,9 @@ reduce_partial_kernel(const double* __restrict__ amp2, const double* __restrict_
     for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n_events;
          e += (int64_t)gridDim.x * blockDim.x) {
         const double w = weight[e];
-        const double x = w * amp2[e] * factor;
+        // an event that failed the cuts contributes exactly 0 whatever its amp2 holds (R26:
+        // a forward photon outside the cuts may have driven amp2 to Inf or NaN, fp32 range included)
+        const double x = (w != 0.0) ? w * amp2[e] * factor : 0.0;
         s1 += x;
         s2 += x * x;
         cnt += (w != 0.0) ? 1.0 : 0.0;
@@ -72,16 +74,16 @@ reduce_final_kernel(const double* __restrict__ partials, int n_partials, double*
 
 }  // namespace
 
-cudaError_t heget_launch_reduce(const heget_ctx* ctx, const double* amp2, const double* weight, int n,
+cudaError_t heget_launch_reduce(double* partials, const double* amp2, const double* weight, int n,
                                 int64_t N, double* out3, cudaStream_t stream, int* launches)
 {
     double nfact = 1.0;
     for (int i = 2; i <= n; ++i) nfact *= (double)i;
     const double factor = kSpinAverage * kColourFactor / nfact;
     *launches = 2;
-    reduce_partial_kernel<<<kReduceBlocks, 256, 0, stream>>>(amp2, weight, N, factor, ctx->d_partials);
+    reduce_partial_kernel<<<kReduceBlocks, 256, 0, stream>>>(amp2, weight, N, factor, partials);
     cudaError_t err = cudaGetLastError();
     if (err != cudaSuccess) return err;
-    reduce_final_kernel<<<1, 256, 0, stream>>>(ctx->d_partials, kReduceBlocks, out3);
+    reduce_final_kernel<<<1, 256, 0, stream>>>(partials, kReduceBlocks, out3);
     return cudaGetLastError();
 }

@@ -62,7 +62,8 @@ def report(tag, rel, passing):
           % (tag, rel.size, int(passing.sum()), p.max(), np.median(p), rel.max(), np.median(rel)))
 
 
-# sizes: several CTAs plus a ragged tail for every n (events per CTA = 256 / 2^n)
+# sizes: several CTAs plus a ragged tail for every n (events per CTA: 64 for n <= 4, one thread per event;
+# 2 at n = 5 and 1 from n = 6 on, one lane per photon-helicity assignment)
 SMALL = {"2gamma": 64 * 5 + 3, "4gamma": 16 * 9 + 5, "6gamma": 4 * 6 + 1, "7gamma": 5, "8gamma": 2}
 if HEAVY:
     SMALL.update({"6gamma": 4 * 30 + 1, "7gamma": 24, "8gamma": 6})

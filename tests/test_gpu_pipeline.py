@@ -38,9 +38,9 @@ def test_gen_events_matches_oracle(hg, name):
     rs = mo[:, 0, 0] + mo[:, 1, 0]                      # scale of every component
     err = np.abs(mg - mo).max(axis=(1, 2)) / rs
     print("\n[gen parity] %s: momenta max rel %.3e median %.3e" % (name, err.max(), np.median(err)))
-    # device log/sincos/pow differ from libm by ulps; RAMBO's conformal boost amplifies an ulp
-    # by gamma^2 = (Q0/M)^2, unbounded for nearly collinear q_i (worst for n = 2), so the bound
-    # is on quantiles plus a loose cap
+    # DESIGN.md reading R25: device log/sincos/pow differ from libm by ulps; RAMBO's conformal boost
+    # amplifies an ulp by gamma^2 = (Q0/M)^2, unbounded for nearly collinear q_i (worst for n = 2,
+    # measured max 1.2e-11), so the bound is on quantiles plus a loose cap
     assert np.median(err) < 1e-15 and np.quantile(err, 0.999) < 1e-12 and err.max() < 1e-9
     # cut decisions: identical except where an observable sits within 1e-9 of a threshold
     same = (wo != 0) == (wg != 0)
@@ -127,6 +127,80 @@ def test_xsec_reduce_matches_oracle_and_is_deterministic(hg, N):
     assert np.array_equal(r1, r2)
     assert r1[2] == ref[2]
     assert abs(r1[0] - ref[0]) <= 1e-13 * abs(ref[0]) and abs(r1[1] - ref[1]) <= 1e-13 * abs(ref[1])
+
+
+def test_xsec_reduce_on_two_streams_does_not_share_scratch(hg):
+    """[dev] calls of one context may run concurrently on different streams (include/heget.h): the
+    block partials of heget_xsec_reduce come from a ring of HEGET_REDUCE_SLOTS buffers, so reductions
+    issued back to back on two streams must each give the result they give alone."""
+    N = 1 << 22
+    rng = np.random.default_rng(7)
+    sets = []
+    for k in range(2):
+        a = torch.from_numpy(rng.uniform(0.5, 2.0, size=N) * 10.0 ** (-7 - 3 * k)).cuda()
+        w = torch.from_numpy(rng.uniform(0.1, 1.0, size=N)).cuda()
+        sets.append((a, w, hg.xsec_reduce(a, w, 4).clone()))
+    torch.cuda.synchronize()
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    for _ in range(20):
+        outs = []
+        for k in (0, 1, 0, 1):
+            with torch.cuda.stream(streams[k]):
+                outs.append((k, hg.xsec_reduce(sets[k][0], sets[k][1], 4)))
+        torch.cuda.synchronize()
+        for k, o in outs:
+            assert torch.equal(o, sets[k][2])
+    # heget_xsec_host has partials of its own: it may follow a reduction that is still running
+    hm, hw = sets[0][0].cpu().pin_memory(), sets[0][1].cpu().pin_memory()
+    mom, _ = oracle.gen_events(2, 2, 64)
+    with torch.cuda.stream(streams[0]):
+        pending = hg.xsec_reduce(sets[1][0], sets[1][1], 4)
+    h3 = hg.xsec_host(torch.from_numpy(mom), torch.ones(64, dtype=torch.float64), FP64)
+    torch.cuda.synchronize()
+    assert torch.equal(pending, sets[1][2]) and torch.isfinite(h3).all()
+
+
+def test_xsec_reduce_ignores_amp2_of_events_that_failed_the_cuts(hg):
+    """DESIGN.md R26: a NaN / Inf amp2 under weight 0 contributes exactly 0 (oracle pinned the same way)."""
+    rng = np.random.default_rng(1)
+    a = rng.uniform(0.5, 2.0, size=5000)
+    w = rng.uniform(0.1, 1.0, size=5000)
+    w[::7] = 0.0
+    clean = hg.xsec_reduce(torch.from_numpy(a).cuda(), torch.from_numpy(w).cuda(), 3).cpu().numpy()
+    b = a.copy()
+    b[::21], b[7::21], b[14::21] = np.nan, np.inf, -np.inf
+    dirty = hg.xsec_reduce(torch.from_numpy(b).cuda(), torch.from_numpy(w).cuda(), 3).cpu().numpy()
+    assert np.array_equal(clean, dirty) and np.all(np.isfinite(dirty))
+    ref = oracle.xsec_reduce(b, w, 3)
+    assert ref[2] == dirty[2] and abs(dirty[0] / ref[0] - 1.0) < 1e-13
+
+
+def test_gen_events_rejects_what_it_cannot_generate():
+    """heget_gen_events: TOYPDF needs tau_min = (n pt_cut)^2 / s inside (0, 1); weight must not be NULL;
+    heget_init rejects non-finite or negative cuts."""
+    import ctypes
+    from paper_0908_4403_b200 import binding
+    lib = binding.load_library()
+    ctx = ctypes.c_void_p()
+    for bad in ((float("nan"), 2.5, 0.4), (20.0, float("inf"), 0.4), (20.0, 2.5, -1.0)):
+        assert lib.heget_init(0, workloads.ALPHA, workloads.Q_U, *bad, ctypes.byref(ctx)) == -1
+    assert lib.heget_init(0, workloads.ALPHA, float("nan"), 20.0, 2.5, 0.4, ctypes.byref(ctx)) == -1
+    h0 = Heget(0, workloads.ALPHA, workloads.Q_U, 0.0, 2.5, 0.4)          # pt_cut = 0: tau_min = 0
+    try:
+        with pytest.raises(Exception):
+            h0.gen_events(1, 4, 16, mode=workloads.TOYPDF, a=14000.0, apply_cuts=False)
+        m, w = h0.gen_events(1, 4, 16, mode=workloads.LOGUNIFORM, a=200.0, b=3000.0, y_max=1.5)   # fine without tau_min
+        assert torch.isfinite(m).all() and torch.isfinite(w).all()
+        cfg = binding.GenCfg(workloads.LOGUNIFORM, 0, 200.0, 3000.0, 1.5)
+        assert lib.heget_gen_events(h0._ctx, 1, 4, ctypes.byref(cfg), 0, 16, m.data_ptr(), None, None) == -1   # weight NULL
+    finally:
+        h0.close()
+    h1 = Heget(0, workloads.ALPHA, workloads.Q_U, 2000.0, 2.5, 0.4)       # 8 x 2 TeV > 14 TeV: tau_min > 1
+    try:
+        with pytest.raises(Exception):
+            h1.gen_events(1, 8, 16, mode=workloads.TOYPDF, a=14000.0, apply_cuts=True)
+    finally:
+        h1.close()
 
 
 @pytest.mark.parametrize("precision", [FP64, FP32])

@@ -136,6 +136,33 @@ def test_xsec_reduce_sums():
     assert out[2] == np.count_nonzero(w)
 
 
+def test_xsec_reduce_ignores_amp2_of_events_that_failed_the_cuts():
+    """DESIGN.md R26: weight 0 means the event is outside the cuts of eq. (9); whatever amp2 holds
+    there (NaN, Inf from a forward photon or an fp32 range excursion) contributes exactly 0."""
+    rng = np.random.default_rng(1)
+    a = rng.uniform(0.5, 2.0, size=64)
+    w = rng.uniform(0.1, 1.0, size=64)
+    w[[3, 17, 40]] = 0.0
+    ref = oracle.xsec_reduce(a, w, 3)
+    b = a.copy()
+    b[3], b[17], b[40] = np.nan, np.inf, -np.inf
+    out = oracle.xsec_reduce(b, w, 3)
+    assert np.array_equal(out, ref) and out[2] == 61
+
+
+@pytest.mark.parametrize("n", [3, 4, 5, 6, 7])
+def test_P9_phase_space_volume_obeys_the_two_body_recursion(n):
+    """Phi_{n+1}(s) = int_0^s dM^2/(2 pi) Phi_n(M^2) Phi_2(s; M, 0): n+1 massless particles = one massless
+    particle recoiling against a cluster of n of mass M, with the two-body volume of masses (M, 0),
+    Phi_2 = (1/8 pi)(1 - M^2/s).  Integrated numerically on the oracle's own Phi_n -- the closed form
+    with its (n-1)!(n-2)! is not restated here."""
+    from scipy.integrate import quad
+    s = 3.7e5
+    integrand = lambda m2: oracle.phase_space_volume(n, m2) * (1.0 - m2 / s) / (8.0 * math.pi) / (2.0 * math.pi)
+    val, err = quad(integrand, 0.0, s, epsabs=0.0, epsrel=1e-12)
+    assert abs(val / oracle.phase_space_volume(n + 1, s) - 1.0) < 1e-10
+
+
 def test_P11_two_photon_partonic_cross_section_closed_form():
     """u ubar -> gamma gamma at sqrt(s_hat) = 1 TeV with |eta| < 2.5 only:
     sigma = 1/(2s) * (1/4)(1/9)(1/2!) * (1/16 pi) * 8 e^4 Q^4 * 4 [ln((1+c)/(1-c)) - c], c = tanh(2.5)
