@@ -2,17 +2,22 @@
 """bench.py -- events/s of the summed squared helicity amplitude of u ubar -> n gamma on B200.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4gamma] [--precision fp64]
-                    [--impl ours|reference] [--no-sweep]
+                    [--impl ours|reference] [--no-sweep] [--no-cpu-baseline]
 
 A step is one pass of the hot path over one batch of the named synthetic workload:
 heget_amp2 (rows a1-a8 of DESIGN.md) followed by heget_xsec_reduce (a9-a10), inputs (momenta,
 weights) resident in HBM.  `e2e` is the same through heget_xsec_host with pinned HOST buffers
-(H2D and D2H copies inside the timed region).  One JSON line is printed by rank 0.
+(H2D and D2H copies inside the timed region).  `pipeline` is the whole chain generated on the
+device: heget_gen_events -> heget_amp2 -> heget_xsec_reduce inside one pair of CUDA events (the
+analogue of the paper's timer, steps 2-6 of PAPER.md:116-122).  `per_config` repeats
+the measurement for n = 2..8 in both precisions.  One JSON line is printed by rank 0.
 """
 import argparse
+import glob
 import json
 import math
 import os
+import re
 import subprocess
 import sys
 import threading
@@ -23,44 +28,47 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 METRIC = "events/s of summed |M|^2 for u ubar->n gamma"
-# dram__bytes_read.sum + dram__bytes_write.sum of one amp2 launch at the config's full size, from
-# the `ncu --set full` captures summarised under profiles/ (n, precision) -> bytes
-NCU_DRAM_BYTES = {(4, "fp64"): 210208512, (4, "fp32"): 210454784, (8, "fp64"): 21140480, (8, "fp32"): 21051648}
-# flop per event of amp2_kernel as ncu counts them over the whole kernel, tables included
-# (smsp__sass_thread_inst_executed_op_{f,d}{fma x2, mul, add}_pred_on of the same captures / events)
-NCU_FLOPS_PER_EVENT = {(4, "fp64"): 8815.0, (4, "fp32"): 7865.1, (8, "fp64"): 1.4349e8, (8, "fp32"): 1.4346e8}
 UNIT = "events/s"
+ALGOS = {"tree": 0, "subset": 1, "two-sided": 2}
+THREAD_MAXN = 4     # n <= 4: one thread per event (csrc/amp2_thread.cu); n >= 5: one lane per helicity assignment
 
+
+def kernel_name(algo, n):
+    if algo == "tree":
+        return "amp2_thread_kernel" if n <= THREAD_MAXN else "amp2_kernel"
+    return {"subset": "amp2_subset_kernel", "two-sided": "amp2_twosided_kernel"}[algo]
+
+
+# ---------------------------------------------------------------------------------------------
+# flop models
 
 def model_flops_per_event(n):
-    """Model C of DESIGN.md: permutation tree with prefix reuse, Weyl form, the 2*2^n non-zero
+    """Model C of SURVEY 8(d): permutation tree with prefix reuse, Weyl form, the 2*2^n non-zero
     helicity assignments; 44 flop per internal node, 24 per leaf (FMA = 2)."""
     internal = sum(math.factorial(n) // math.factorial(n - l) for l in range(1, n))
     return 2 * 2 ** n * (44 * internal + 24 * math.factorial(n))
 
 
 def executed_flops_per_event(n, precision="fp32"):
-    """What amp2_kernel executes: 2^n lanes (sigma_1 = +1 only, doubled by
-    parity), tables excluded.
-    n >= 5 (v9, factorised nodes psi = z v, csrc/amp2_chain.cuh): every ordered prefix of up to n-3
-    photons is rho (4 FMA) + the vector v of the node (5 FMA + 1 MUL) + the accumulation rho A
-    (4 FMA) = 27 flop, every prefix of n-2 photons (its two remaining orderings closed by the
-    per-event table of closing dots) rho + accumulation = 16 flop.
-    n = 4 (v8): one fvixx0 node = 16 FMA + 4 MUL = 36 flop for every ordered prefix of up to n-2
-    photons and one dot product with the pair closing table, 8 FMA = 16 flop, per prefix of n-2
-    photons; the first two tree levels once per event (48 entries psi_2 in factorised form, 42 flop
-    each) instead of once per lane (16 nodes).  n = 2, 3 (v7): 36 flop per node and two vertex + closing-table dots,
-    2 x (16 + 16) = 64 flop, per prefix of n-2 photons.  Cross-checked against ncu's
-    sass_thread_inst_executed_op_{f,d}{fma,mul,add} counters in profiles/."""
+    """What the tree kernels execute per event, tables excluded.
+    n >= 5 (lane per helicity assignment, factorised nodes psi = z v, csrc/amp2_chain.cuh): 2^n lanes;
+    every ordered prefix of up to n-3 photons is rho (4 FMA) + the vector v of the node (5 FMA + 1 MUL)
+    + the accumulation rho A (4 FMA) = 27 flop; a prefix of n-2 photons (its two remaining orderings
+    closed by the per-event table of closing dots) is rho + accumulation = 16 flop.
+    n <= 4 (thread per event, csrc/amp2_thread.cu): nodes are shared between helicity assignments (a
+    prefix is evaluated once per helicity assignment of ITS photons): n = 4: 8 vectors v1 (11 flop),
+    24 vectors v2 (11), 48 rho (8), 48 scalings/accumulations of psi_2 (16), 96 closing dots (16);
+    n = 3: 6 vectors (11), 24 dots (16 + 2); n = 2: the closing rows only (counted with the tables).
+    The kernels' whole count, tables included, is read from the SASS (sass_flops_per_event) or from the
+    ncu summaries under profiles/."""
     if n >= 5:
         upper = sum(math.factorial(n) // math.factorial(n - l) for l in range(1, n - 2))
         return 2 ** n * (27 * upper + 16 * (math.factorial(n) // 2))
-    upper = sum(math.factorial(n) // math.factorial(n - l) for l in range(1, n - 1))
-    closing = 16 if n >= 4 else 64
-    flops = 2 ** n * (36 * upper + closing * (math.factorial(n) // 2))
     if n == 4:
-        flops -= 2 ** n * 16 * 36 - 48 * 42   # 48 entries psi_2 = rho v per event, 42 flop each (factorised form)
-    return flops
+        return 8 * 11 + 24 * 11 + 48 * 8 + 48 * 16 + 96 * 16
+    if n == 3:
+        return 6 * 11 + 24 * 18
+    return 0
 
 
 def _binom(n, k):
@@ -91,14 +99,88 @@ def executed_flops_per_event_algo(n, algo, precision="fp32"):
     return 2 ** n * per_lane + table
 
 
-ALGOS = {"tree": 0, "subset": 1, "two-sided": 2}
-KERNEL_NAME = {"tree": "amp2_kernel", "subset": "amp2_subset_kernel", "two-sided": "amp2_twosided_kernel"}
+_SASS_CACHE = {}
+
+
+def sass_flops_per_event(n, precision):
+    """Flops per event of the thread-per-event kernels (n <= 4), counted in the SASS of the library
+    that is loaded: those kernels are straight-line code executed once per event, so the static count
+    of {D,F}FMA (x2), {D,F}MUL, {D,F}ADD IS the executed count, tables included.  None if cuobjdump is
+    not available or the kernel has a loop."""
+    if n > THREAD_MAXN:
+        return None
+    key = (n, precision)
+    if key in _SASS_CACHE:
+        return _SASS_CACHE[key]
+    from paper_0908_4403_b200 import binding
+    val = None
+    try:
+        out = subprocess.run(["cuobjdump", "-sass", binding.LIB_PATH], capture_output=True, text=True, timeout=120).stdout
+        want = "amp2_thread_kernelILi%dE%s" % (n, "d" if precision == "fp64" else "f")
+        body, on = [], False
+        for line in out.splitlines():
+            if "Function :" in line:
+                on = want in line
+            elif on:
+                body.append(line)
+        ops = [m.group(1) for m in (re.match(r"\s+/\*[0-9a-f]{4,}\*/\s+(?:@!?U?P\d\s+)?([A-Z0-9_.]+)", l) for l in body) if m]
+        if ops and not any(o.startswith("BRA") for o in ops[:-2]):
+            count = lambda p: sum(1 for o in ops if o.split(".")[0] == p)
+            val = float(2 * (count("DFMA") + count("FFMA")) + count("DMUL") + count("FMUL") + count("DADD") + count("FADD"))
+    except Exception:
+        val = None
+    _SASS_CACHE[key] = val
+    return val
+
+
+def ncu_summary(config, precision, kernel, measured_ms, events):
+    """The committed `ncu --set full` summary of this kernel under profiles/ (newest round first):
+    counted flops per event, DRAM bytes per launch and the kernel time of the capture.  The summary
+    describes the binary it was captured from: it is used only if it names the kernel that runs now
+    and its duration agrees with the one measured here within 5 %; otherwise the status says why and
+    the caller falls back to what it can measure itself."""
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_amp2_%s_%s.txt" % (config, precision))), reverse=True)
+    if not files:
+        return {"status": "no summary under profiles/ for %s %s" % (config, precision)}
+    text = open(files[0]).read()
+    name = os.path.relpath(files[0], ROOT)
+    m_kernel = re.search(r"^kernel: .*?(\w+)<", text, re.M)
+    m_time = re.search(r"gpu__time_duration\.sum\s+([0-9.,]+)\s*(us|ms|ns|s)\b", text)
+    m_flop = re.search(r"=\s*([0-9.eE+]+) flop per event", text)
+    m_ev = re.search(r"/\s*(\d+) events", text)
+    scale = {"ns": 1e-6, "us": 1e-3, "ms": 1.0, "s": 1e3}
+    unit = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    dram = 0.0
+    for key in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+        m = re.search(re.escape(key) + r"\s+([0-9.,]+)\s*(\w+)", text)
+        if not m or m.group(2) not in unit:
+            return {"status": "STALE: %s has no %s" % (name, key), "file": name}
+        dram += float(m.group(1).replace(",", "")) * unit[m.group(2)]
+    if not (m_kernel and m_time and m_flop and m_ev):
+        return {"status": "STALE: %s is not a summary this parser understands" % name, "file": name}
+    ms = float(m_time.group(1).replace(",", "")) * scale[m_time.group(2)]
+    out = {"file": name, "kernel": m_kernel.group(1), "kernel_ms": ms, "flops_per_event": float(m_flop.group(1)),
+           "dram_bytes": dram, "events": int(m_ev.group(1))}
+    if out["kernel"] != kernel:
+        out["status"] = "STALE: %s is a capture of %s, the kernel that runs is %s" % (name, out["kernel"], kernel)
+    elif out["events"] != events:
+        out["status"] = "STALE: %s was captured on %d events, this run has %d" % (name, out["events"], events)
+    elif abs(ms / measured_ms - 1.0) > 0.05:
+        out["status"] = "STALE: %s says %.4f ms, measured here %.4f ms (> 5 %% apart)" % (name, ms, measured_ms)
+    else:
+        out["status"] = "ok"
+    if out["status"] != "ok":
+        sys.stderr.write("bench.py: " + out["status"] + "\n")
+    return out
 
 
 def theoretical_peak(precision, sm_count, sm_max_mhz):
     lanes = 128 if precision == "fp32" else 64       # FP32 / FP64 FMA lanes per SM on B200
     return sm_count * lanes * 2 * sm_max_mhz * 1e6
 
+
+# ---------------------------------------------------------------------------------------------
+# clocks
 
 class ClockSampler:
     """SM clock and throttle reasons sampled DURING the timed region: through NVML in-process
@@ -171,17 +253,22 @@ class ClockSampler:
                 "reasons": [n for n in self.NAMES if n in self.reasons], "samples": len(sm), "source": self.source}
 
 
+# ---------------------------------------------------------------------------------------------
+# CPU baseline: the oracle as it stands, on the host cores
+
+# rough oracle<double> cost per event in core-seconds (sizes the one-second pilot only)
+ORACLE_CORE_S = {2: 2e-6, 3: 2.5e-5, 4: 5e-4, 5: 1e-2, 6: 0.4, 7: 7.0, 8: 130.0}
+
+
 def oracle_sample_events(cfg, seconds_budget=12.0):
     """How many events of this config the oracle is timed on: a BOUNDED sample sized for about
-    `seconds_budget` seconds of wall time on this host (10-30 s of CPU work on all its cores),
-    from a one-second pilot run of the oracle itself."""
+    `seconds_budget` seconds of wall time on this host, from a pilot run of the oracle itself."""
     cores = os.cpu_count() or 1
-    per_event_core_s = {2: 2e-6, 3: 2.5e-5, 4: 1e-4, 5: 1.5e-3, 6: 2.5e-2, 7: 0.4, 8: 6.0}[cfg["n"]]
-    pilot = max(min(int(1.0 * cores / per_event_core_s), cfg["N"]), 1)
+    pilot = max(min(int(1.0 * cores / ORACLE_CORE_S[cfg["n"]]), cfg["N"]), 1)
+    if ORACLE_CORE_S[cfg["n"]] / cores > seconds_budget / 2:
+        return 1      # one event is already most of the budget (the oracle spreads its helicity assignments over the cores)
     rate, _, _ = time_oracle(cfg, pilot)
-    want = int(rate * seconds_budget)
-    # at least one event (the oracle spreads a single event's helicity assignments over the cores)
-    return max(min(want, cfg["N"]), 1)
+    return max(min(int(rate * seconds_budget), cfg["N"]), 1)
 
 
 def time_oracle(cfg, n_events):
@@ -195,6 +282,13 @@ def time_oracle(cfg, n_events):
     oracle.amp2(mom)
     dt = time.perf_counter() - t0
     return n_events / dt, dt, oracle.num_threads()
+
+
+def cpu_baseline(name, cfg, seconds_budget):
+    n_ev = oracle_sample_events(cfg, seconds_budget)
+    v, dt, cores = time_oracle(cfg, n_ev)
+    return {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": "first %d of %d events of %s, oracle<double>, %.1f s" % (n_ev, cfg["N"], name, dt)}
 
 
 def run_reference(args):
@@ -222,33 +316,7 @@ def run_reference(args):
         "gpu_launches": 0}))
 
 
-def time_config(hg, torch, name, precision, steps, warmup, flush, first_event, n_local, algo=0):
-    """Device-timed steps of amp2 + xsec_reduce on resident inputs.  Returns per-step ms (whole
-    step) and the amp2 kernel's own ms, both from CUDA events on the launching stream."""
-    from paper_0908_4403_b200 import FP32, FP64, workloads
-    cfg = workloads.CONFIGS[name]
-    prec = FP64 if precision == "fp64" else FP32
-    mom, w = hg.gen_events(cfg["seed"], cfg["n"], n_local, mode=cfg["mode"], a=cfg["a"], b=cfg["b"],
-                           y_max=cfg["y_max"], apply_cuts=cfg["apply_cuts"], first_event=first_event)
-    amp2 = torch.empty(n_local, dtype=torch.float64, device=hg.device)
-    out3 = torch.empty(3, dtype=torch.float64, device=hg.device)
-
-    def step(ev=None):
-        if ev:
-            ev[0].record()
-        hg.amp2(mom, prec, out=amp2, algo=algo)
-        if ev:
-            ev[1].record()
-        hg.xsec_reduce(amp2, w, cfg["n"], out3=out3)
-        if ev:
-            ev[2].record()
-
-    for _ in range(warmup):
-        step()
-    torch.cuda.synchronize()
-    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(steps)]
-    return mom, w, out3, step, evs, flush
-
+# ---------------------------------------------------------------------------------------------
 
 def main():
     ap = argparse.ArgumentParser()
@@ -283,68 +351,104 @@ def main():
     hg = Heget(local_rank, workloads.ALPHA, workloads.Q_U, workloads.PT_CUT, workloads.ETA_CUT, workloads.DR_CUT)
     cfg = workloads.CONFIGS[args.config]
     n = cfg["n"]
-    # weak scaling: every rank processes the full per-GPU batch of the config, on its own
-    # contiguous range of global event indices (no data-path collective; the three sums of
-    # the reduction are all-reduced once per step)
-    n_local = cfg["N"]
-    first_event = rank * n_local
     flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device=hg.device)   # > 126 MB L2
+    PREC = {"fp64": FP64, "fp32": FP32}
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    def timed_run(name, precision, steps, warmup, algo=0):
-        c = workloads.CONFIGS[name]
-        nl = c["N"]
-        mom, w, out3, step, evs, _ = time_config(hg, torch, name, precision, steps, warmup, None, rank * nl, nl, algo)
-        barrier()
-        for ev in evs:
-            flush_buf.zero_()                                  # L2 flush, outside the timed events
-            step(ev)
-            if world > 1:
-                dist.all_reduce(out3)
-        barrier()
-        step_ms = [e[0].elapsed_time(e[2]) for e in evs]
-        amp_ms = [e[0].elapsed_time(e[1]) for e in evs]
-        return sum(step_ms), sum(amp_ms) / len(amp_ms), min(amp_ms), out3.cpu().numpy(), nl
+    def gen(c, nl, first, momenta=None, weight=None):
+        return hg.gen_events(c["seed"], c["n"], nl, mode=c["mode"], a=c["a"], b=c["b"], y_max=c["y_max"],
+                             apply_cuts=c["apply_cuts"], first_event=first, momenta=momenta, weight=weight)
 
+    def timed_run(name, precision, steps, warmup, algo=0, pipeline=False):
+        """Device-timed steps on resident inputs: heget_amp2 + heget_xsec_reduce (+ the all-reduce of
+        the three sums for world > 1), or with pipeline=True heget_gen_events + both, CUDA events on the
+        launching stream.  Weak scaling: every rank processes the config's full per-GPU batch on its own
+        contiguous range of global event indices.  Returns total ms over the steps, the mean and
+        best amp2-kernel ms, the three sums and the events per rank."""
+        c = workloads.CONFIGS[name]
+        nl, first = c["N"], rank * c["N"]
+        mom, w = gen(c, nl, first)
+        amp2 = torch.empty(nl, dtype=torch.float64, device=hg.device)
+        out3 = torch.empty(3, dtype=torch.float64, device=hg.device)
+
+        def step(ev=None):
+            if ev:
+                ev[0].record()
+            if pipeline:
+                gen(c, nl, first, mom, w)
+            if ev:
+                ev[1].record()
+            hg.amp2(mom, PREC[precision], out=amp2, algo=algo)
+            if ev:
+                ev[2].record()
+            hg.xsec_reduce(amp2, w, c["n"], out3=out3)
+            if world > 1:
+                dist.all_reduce(out3)              # the only exchange of the path, inside the timed window
+            if ev:
+                ev[3].record()
+
+        for _ in range(warmup):
+            step()
+        barrier()
+        evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(steps)]
+        for ev in evs:
+            flush_buf.zero_()                      # L2 flush, outside the timed events
+            step(ev)
+        barrier()
+        step_ms = [e[0].elapsed_time(e[3]) for e in evs]
+        amp_ms = [e[1].elapsed_time(e[2]) for e in evs]
+        gen_ms = [e[0].elapsed_time(e[1]) for e in evs]
+        return {"total_ms": sum(step_ms), "step_ms": sum(step_ms) / steps, "amp_ms": sum(amp_ms) / steps,
+                "amp_ms_best": min(amp_ms), "gen_ms": sum(gen_ms) / steps, "sums": out3.cpu().numpy(), "events": nl}
+
+    def max_over_ranks(x):
+        if world > 1:
+            t = torch.tensor([x], dtype=torch.float64, device=hg.device)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            return t.item()
+        return x
+
+    # ---- headline: amp2 + reduce on resident inputs
     launches0 = hg.launch_count()
     sampler = ClockSampler(local_rank)
     sampler.start()
-    total_ms, amp_ms, amp_ms_best, sums, nl = timed_run(args.config, args.precision, args.steps, args.warmup,
-                                                         algo=ALGOS[args.algo])
+    head = timed_run(args.config, args.precision, args.steps, args.warmup, algo=ALGOS[args.algo])
     clocks = sampler.stop()
     launches = hg.launch_count() - launches0 - 3 * args.warmup - 1   # minus warm-up steps and the generator
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=hg.device)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = t.item()
+    nl = head["events"]
+    total_ms = max_over_ranks(head["total_ms"])
     value = world * nl * args.steps / (total_ms * 1e-3)
+    amp_ms, amp_ms_best, sums = head["amp_ms"], head["amp_ms_best"], head["sums"]
 
-    # end to end through the host-buffer entry point (pinned host inputs, H2D + D2H inside)
-    mom_d, w_d = hg.gen_events(cfg["seed"], n, nl, mode=cfg["mode"], a=cfg["a"], b=cfg["b"], y_max=cfg["y_max"],
-                               apply_cuts=cfg["apply_cuts"], first_event=first_event)
+    # ---- pipeline: gen + amp2 + reduce in one event pair (device-generated inputs, nothing crosses PCIe)
+    pipe = timed_run(args.config, args.precision, max(1, min(args.steps, 5)), 3, algo=ALGOS[args.algo], pipeline=True)
+    pipe_ms = max_over_ranks(pipe["step_ms"])
+
+    # ---- end to end through the host-buffer entry point (pinned host inputs, H2D + D2H inside)
+    mom_d, w_d = gen(cfg, nl, rank * nl)
     mom_h = torch.empty(mom_d.shape, dtype=torch.float64).pin_memory()
     w_h = torch.empty(w_d.shape, dtype=torch.float64).pin_memory()
     mom_h.copy_(mom_d)
     w_h.copy_(w_d)
     out3_h = torch.empty(3, dtype=torch.float64).pin_memory()
-    prec = FP64 if args.precision == "fp64" else FP32
-    for _ in range(2):
+    prec = PREC[args.precision]
+    for _ in range(3):       # warm-up, and the staging buffers of heget_xsec_host are allocated here
         hg.xsec_host(mom_h, w_h, prec, out3=out3_h)
     barrier()
     e2e_steps = max(1, min(args.steps, 5))
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
         hg.xsec_host(mom_h, w_h, prec, out3=out3_h)
+        if world > 1:
+            t3 = out3_h.to(hg.device)
+            dist.all_reduce(t3)
+            out3_h.copy_(t3)
     barrier()
-    e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device=hg.device)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = t.item()
+    e2e_s = max_over_ranks(time.perf_counter() - t0)
     e2e_value = world * nl * e2e_steps / e2e_s
 
     if rank != 0:
@@ -352,45 +456,53 @@ def main():
             dist.destroy_process_group()
         return
 
-    # roofline of the dominant kernel (amp2): plain-ALU bound.  `achieved` = flops the kernel
-    # executes (the ncu-counted figure is the %peak figure) over its own time;
-    # model C (the survey's algorithmic count, which ignores the parity relation and the
-    # normalised E' entries) over the same time is given beside it as the cross-check.
-    peak_measured = hg.fma_peak(prec, 0)
-    peak_3reg = hg.fma_peak(prec, 1)
-    peak_node = hg.fma_peak(prec, 2)
+    # ---- roofline of the dominant kernel (amp2): plain-ALU bound.  `achieved` = flops the kernel
+    # executes (the ncu-counted figure is the %peak figure) over its own time, measured
+    # here with CUDA events; model C (the survey's algorithmic count, which ignores the parity relation,
+    # the normalised E' entries and the sharing of prefixes between helicity assignments) over the
+    # same time is given beside it as the cross-check.
+    props = torch.cuda.get_device_properties(local_rank)
     sm_max = clocks["sm_max_mhz"] or 1965.0
-    peak_theory = theoretical_peak(args.precision, torch.cuda.get_device_properties(local_rank).multi_processor_count, sm_max)
+    peaks = {p: {"measured": hg.fma_peak(PREC[p], 0), "three_reg": hg.fma_peak(PREC[p], 1), "node": hg.fma_peak(PREC[p], 2),
+                 "theory": theoretical_peak(p, props.multi_processor_count, sm_max)} for p in ("fp64", "fp32")}
+
+    def flops_of(name, nph, precision, algo, ms, events):
+        """(flops per event, source, ncu summary or None) for one kernel of this run."""
+        summ = ncu_summary(name, precision, kernel_name(algo, nph), ms, events) if algo == "tree" else None
+        if summ and summ["status"] == "ok":
+            return summ["flops_per_event"], "ncu-counted over the whole kernel, tables included (%s)" % summ["file"], summ
+        sass = sass_flops_per_event(nph, precision) if algo == "tree" else None
+        if sass:
+            return sass, "counted in the SASS of the loaded library (straight-line kernel, one pass per event, tables included)", summ
+        return (executed_flops_per_event_algo(nph, algo, precision),
+                "executed-instruction model of the tree, tables (< 1 % from 6 photons on) excluded", summ)
+
+    pk = peaks[args.precision]
+    fpe, fsrc, summ = flops_of(args.config, n, args.precision, args.algo, amp_ms, nl)
     tree_model = executed_flops_per_event_algo(n, args.algo, args.precision)
-    counted = NCU_FLOPS_PER_EVENT.get((n, args.precision)) if args.algo == "tree" else None
-    flops_per_event = counted if counted is not None else tree_model
-    achieved = flops_per_event * nl / (amp_ms * 1e-3)
+    achieved = fpe * nl / (amp_ms * 1e-3)
     model_c = model_flops_per_event(n) * nl / (amp_ms * 1e-3)
-    roofline = {"bound": "alu", "achieved": achieved / 1e12, "peak": peak_measured / 1e12, "unit": "TFLOP/s",
-                "frac": achieved / peak_measured, "traffic": NCU_DRAM_BYTES.get((n, args.precision)) if args.algo == "tree" else None,
-                "kernel": "%s<%d,%s>" % (KERNEL_NAME[args.algo], n, "double" if prec == FP64 else "float"),
+    bytes_alg = nl * ((n + 2) * 32 + 8)
+    roofline = {"bound": "alu", "achieved": achieved / 1e12, "peak": pk["measured"] / 1e12, "unit": "TFLOP/s",
+                "frac": achieved / pk["measured"],
+                "traffic": summ["dram_bytes"] if summ and summ["status"] == "ok" else None,
+                "kernel": "%s<%d,%s>" % (kernel_name(args.algo, n), n, "double" if prec == FP64 else "float"),
                 "kernel_ms": amp_ms, "kernel_ms_best": amp_ms_best,
-                "flops_per_event": flops_per_event,
-                "flops_source": ("ncu-counted over the whole kernel, tables included (profiles/)" if counted is not None
-                                 else "executed-instruction model of the tree, tables (< 1 % from 6 photons on) excluded"),
-                "flops_per_event_executed": tree_model,
+                "flops_per_event": fpe, "flops_source": fsrc,
+                "ncu_summary": ({k: summ[k] for k in ("status", "file", "kernel_ms") if k in summ} if summ else None),
+                "flops_per_event_tree_model": tree_model,
                 "tree_model_tflops": tree_model * nl / (amp_ms * 1e-3) / 1e12,
                 "peak_source": "heget_fma_peak on this GPU: FMA with constant-bank operands "
                                "(MEASURED_PEAKS.json has no non-tensor figure)",
-                "peak_theoretical": peak_theory / 1e12, "frac_of_theoretical": achieved / peak_theory,
-                "peak_three_register_fma": peak_3reg / 1e12, "peak_node_pattern": peak_node / 1e12,
-                "frac_of_node_pattern": achieved / peak_node,
-                "model_c_tflops": model_c / 1e12, "model_c_frac": model_c / peak_measured,
+                "peak_theoretical": pk["theory"] / 1e12, "frac_of_theoretical": achieved / pk["theory"],
+                "peak_three_register_fma": pk["three_reg"] / 1e12, "peak_node_pattern": pk["node"] / 1e12,
+                "frac_of_node_pattern": achieved / pk["node"],
+                "model_c_tflops": model_c / 1e12, "model_c_frac": model_c / pk["measured"],
+                "algorithmic_bytes": bytes_alg, "hbm_gbs": bytes_alg / (amp_ms * 1e-3) / 1e9,
                 "frac_note": "frac counts EXECUTED flops (what ncu counts); model_c_frac counts SURVEY 8(d)'s fixed "
-                             "algorithmic figure (model C) over the same time.  Work removed by the parity relation and "
-                             "by re-associating or sharing factors lowers frac while events/s and model_c_frac rise "
-                             "(4 gamma fp64: v3 1.48 ms, frac 0.56 -> v7 1.02 ms, 0.48 -> v8 0.745 ms, 0.41 -> v9 0.70 ms, 0.39)",
-                "flops_model": "executed: n = 4: 2^n lanes x (36 flop per tree node down to depth n-2 + 16 per pair of last "
-                               "orderings, one dot with the pair closing table); n >= 5: 2^n lanes x (27 flop per factorised "
-                               "node down to depth n-3 + 16 per node of n-2 photons), see executed_flops_per_event; model C (SURVEY 8(d)): 2*2^n x (44 per node "
-                               "+ 24 per leaf), 3-5x the executed count because the kernel evaluates sigma_1=+1 only "
-                               "(parity), uses normalised polarisation blocks and contracts the last two vertices and "
-                               "the last propagator of both final orderings into a per-event table"}
+                             "algorithmic figure (model C) over the same time.  Work removed by the parity relation, by "
+                             "sharing prefixes between helicity assignments and by re-associating factors lowers frac "
+                             "while events/s and model_c_frac rise"}
 
     result = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
               "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
@@ -402,40 +514,54 @@ def main():
               "clocks": clocks,
               "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(mom_h.numel() * 8 + w_h.numel() * 8),
                       "d2h_bytes_per_step": 24, "steps": e2e_steps},
+              "pipeline": {"value": world * nl / (pipe_ms * 1e-3), "unit": UNIT, "ms_per_step": pipe_ms,
+                           "gen_ms": pipe["gen_ms"], "amp2_ms": pipe["amp_ms"],
+                           "what": "heget_gen_events + heget_amp2 + heget_xsec_reduce inside one CUDA-event pair"},
               "gpu_launches": int(launches),
               "roofline": roofline,
               "xsec": {"sum_wA": float(sums[0]), "sum_wA2": float(sums[1]), "n_pass": float(sums[2])}}
 
     if not args.no_cpu_baseline:
-        n_ev = oracle_sample_events(cfg)
-        v, dt, cores = time_oracle(cfg, n_ev)
-        result["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                  "sample": "first %d of %d events of %s, oracle<double>, %.1f s" % (n_ev, cfg["N"], args.config, dt)}
+        result["cpu_baseline"] = cpu_baseline(args.config, cfg, 12.0)
 
     if not args.no_sweep and world == 1:
         table = []
         for name in workloads.ORDER:
+            c = workloads.CONFIGS[name]
+            nph = c["n"]
+            cpu = None if args.no_cpu_baseline else cpu_baseline(name, c, 3.0)
             for precision in ("fp32", "fp64"):
-                _, a_ms, a_best, _, nn = timed_run(name, precision, 3, 3)
-                nph = workloads.CONFIGS[name]["n"]
-                pk = peak_measured if precision == args.precision else hg.fma_peak(FP64 if precision == "fp64" else FP32)
-                ach = executed_flops_per_event(nph, precision) * nn / (a_ms * 1e-3)
-                for algo_id, algo_name, note in (
-                        (1, "subset", "HEGET_ALGO_SUBSET (heget_amp2_algo): not the permutation tree, own flop count"),
-                        (2, "two-sided", "HEGET_ALGO_TREE2 (heget_amp2_algo): tree from u to depth n-4, closed with "
-                                         "row vectors chained from ubar; own flop count")):
-                    _, s_ms, _, _, _ = timed_run(name, precision, 3, 3, algo=algo_id)
-                    s_fl = executed_flops_per_event_algo(nph, algo_name, precision) * nn / (s_ms * 1e-3)
-                    table.append({"workload": name, "n": nph, "precision": precision, "events": nn, "algo": algo_name,
-                                  "amp2_ms": s_ms, "events_per_s": nn / (s_ms * 1e-3),
-                                  "executed_tflops": s_fl / 1e12, "frac_of_measured_peak": s_fl / pk, "note": note})
-                table.append({"workload": name, "n": nph, "precision": precision, "events": nn, "algo": "tree",
-                              "amp2_ms": a_ms, "events_per_s": nn / (a_ms * 1e-3),
-                              "executed_tflops": ach / 1e12, "frac_of_measured_peak": ach / pk,
-                              "model_c_tflops": model_flops_per_event(nph) * nn / (a_ms * 1e-3) / 1e12})
+                pkk = peaks[precision]
+                for algo_name, note in (
+                        ("tree", None),
+                        ("subset", "HEGET_ALGO_SUBSET (heget_amp2_algo): not the permutation tree, own flop count"),
+                        ("two-sided", "HEGET_ALGO_TREE2 (heget_amp2_algo): tree from u to depth n-4, closed with "
+                                      "row vectors chained from ubar; own flop count")):
+                    r = timed_run(name, precision, 3, 3, algo=ALGOS[algo_name])
+                    ms, nn = r["amp_ms"], r["events"]
+                    row = {"workload": name, "n": nph, "precision": precision, "events": nn, "algo": algo_name,
+                           "amp2_ms": ms, "amp2_ms_best": r["amp_ms_best"], "events_per_s": nn / (ms * 1e-3)}
+                    model = executed_flops_per_event_algo(nph, algo_name, precision)
+                    row["executed_tflops"] = model * nn / (ms * 1e-3) / 1e12
+                    if algo_name == "tree":
+                        f, src, s = flops_of(name, nph, precision, "tree", ms, nn)
+                        p = timed_run(name, precision, 3, 3, pipeline=True)
+                        row.update({"counted_tflops": f * nn / (ms * 1e-3) / 1e12, "flops_per_event": f, "flops_source": src,
+                                    "frac_of_measured_peak": f * nn / (ms * 1e-3) / pkk["measured"],
+                                    "frac_of_theoretical_peak": f * nn / (ms * 1e-3) / pkk["theory"],
+                                    "model_c_tflops": model_flops_per_event(nph) * nn / (ms * 1e-3) / 1e12,
+                                    "hbm_gbs": nn * ((nph + 2) * 32 + 8) / (ms * 1e-3) / 1e9,
+                                    "pipeline_ms": p["step_ms"], "gen_ms": p["gen_ms"],
+                                    "pipeline_events_per_s": nn / (p["step_ms"] * 1e-3)})
+                        if cpu:
+                            row["cpu_baseline"] = cpu
+                    else:
+                        row.update({"frac_of_measured_peak": model * nn / (ms * 1e-3) / pkk["measured"], "note": note})
+                    table.append(row)
         result["per_config"] = table
+        result["peaks_tflops"] = {p: {k: v / 1e12 for k, v in d.items()} for p, d in peaks.items()}
+        result["hbm_peak_gbs"] = _hbm_peak()
 
-    if not args.no_sweep and world == 1:
         # NEXT-1 entry points on the headline workload: one drawn helicity per event, Fig. 2 histogram
         ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
         val, _ = hg.amp2_sampled(cfg["seed"], mom_d, prec)
@@ -447,40 +573,21 @@ def main():
         hg.histogram(mom_d, val, 0, 0.0, 1500.0, 60)
         ev[2].record()
         torch.cuda.synchronize()
-        ev2 = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
-        hg.list2(cfg["seed"], mom_d, prec)
-        torch.cuda.synchronize()
-        ev2[0].record()
-        hg.list2(cfg["seed"], mom_d, prec)
-        ev2[1].record()
-        torch.cuda.synchronize()
-        # the paper's arithmetic for the headline quantity on this GPU: List 2 called for all 4*2^n
-        # helicity assignments per thread (model A of SURVEY 8(d)); bounded to n <= 6
-        if n <= 6:
-            n_pd = nl if n <= 4 else nl // 64
-            ev3 = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
-            sub = mom_d[:n_pd].contiguous()
-            hg.list2_sum(sub, prec)
-            torch.cuda.synchronize()
-            ev3[0].record()
-            hg.list2_sum(sub, prec)
-            ev3[1].record()
-            torch.cuda.synchronize()
-            pd_ms = ev3[0].elapsed_time(ev3[1])
-            result["paper_design"] = {"events_per_s": n_pd / (pd_ms * 1e-3), "ms": pd_ms, "events": n_pd,
-                                      "note": "heget_list2_sum: the paper's List 2 program (thread per event, "
-                                              "4-component, no prefix reuse, no parity) looped over all helicity "
-                                              "assignments, same GPU, same precision, same momenta"}
-        result["next1"] = {"paper_list2_ms": ev2[0].elapsed_time(ev2[1]),
-                           "paper_list2_events_per_s": nl / (ev2[0].elapsed_time(ev2[1]) * 1e-3),
-                           "paper_list2_note": "heget_list2: the paper's List 2 program (thread per event, 4-component, "
-                                               "no reuse) on this GPU, same estimator as amp2_sampled",
-                           "amp2_sampled_ms": ev[0].elapsed_time(ev[1]),
+        result["next1"] = {"amp2_sampled_ms": ev[0].elapsed_time(ev[1]),
                            "amp2_sampled_events_per_s": nl / (ev[0].elapsed_time(ev[1]) * 1e-3),
                            "histogram_ms": ev[1].elapsed_time(ev[2]), "events": nl, "precision": args.precision}
 
     print(json.dumps(result))
     hg.close()
+
+
+def _hbm_peak():
+    """Measured HBM copy rate of this pool's B200s (driver-written MEASURED_PEAKS.json), else the
+    fallback of the profiling guide."""
+    try:
+        return {"value": json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"], "source": "MEASURED_PEAKS.json"}
+    except Exception:
+        return {"value": 6540.0, "source": "fallback: B200_PROFILING.md"}
 
 
 if __name__ == "__main__":

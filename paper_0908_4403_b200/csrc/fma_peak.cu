@@ -90,7 +90,13 @@ cudaError_t run(const heget_ctx* ctx, int pattern, double* flops_per_s, int* lau
     T* sink = nullptr;
     cudaError_t err = cudaMalloc(&sink, sizeof(T) * 1024);
     if (err != cudaSuccess) return err;
-    cudaMemset(sink, 0, sizeof(T) * 1024);  // operands of patterns 1, 2 (zeros: values do not matter)
+    {   // operands of patterns 1, 2: non-trivial values of order one (all-zero data would toggle fewer bits,
+        // draw less power and could clock higher than real operands do), contracting so the chains stay finite
+        T host[1024];
+        for (int i = 0; i < 1024; ++i) host[i] = (T)(0.25 + 0.5 * ((i * 2654435761u) % 1000) / 1000.0) * ((i & 1) ? (T)1 : (T)-1);
+        err = cudaMemcpy(sink, host, sizeof(host), cudaMemcpyHostToDevice);
+        if (err != cudaSuccess) { cudaFree(sink); return err; }
+    }
     cudaEvent_t t0, t1;
     cudaEventCreate(&t0);
     cudaEventCreate(&t1);

@@ -18,7 +18,6 @@ from paper_0908_4403_b200 import ALGO_SUBSET, ALGO_TREE, ALGO_TREE2, FP32, FP64,
 pytestmark = pytest.mark.gpu
 
 TOL64, TOL32 = 1e-12, 1e-4
-HEAVY = os.environ.get("HEGET_TEST_HEAVY", "0") == "1"
 
 
 @pytest.fixture(scope="module")
@@ -64,9 +63,22 @@ def report(tag, rel, passing):
 
 # sizes: several CTAs plus a ragged tail for every n (events per CTA: 64 for n <= 4, one thread per event;
 # 2 at n = 5 and 1 from n = 6 on, one lane per photon-helicity assignment)
-SMALL = {"2gamma": 64 * 5 + 3, "4gamma": 16 * 9 + 5, "6gamma": 4 * 6 + 1, "7gamma": 5, "8gamma": 2}
-if HEAVY:
-    SMALL.update({"6gamma": 4 * 30 + 1, "7gamma": 24, "8gamma": 6})
+SMALL = {"2gamma": 64 * 5 + 3, "3gamma": 64 * 2 + 7, "4gamma": 16 * 9 + 5, "5gamma": 2 * 20 + 3, "6gamma": 4 * 6 + 1,
+         "7gamma": 9, "8gamma": 5}
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def golden_events(name, count):
+    """For n >= 6 the inputs and oracle<long double> values come from the stored golden sets
+    (tests/golden/make_amp2_golden.py; all of them are compared in test_gpu_golden.py): the first
+    `count - 1` cut-passing events of the config and its first failing one."""
+    path = os.path.join(GOLDEN, "amp2_%s.npz" % name)
+    if not os.path.exists(path):
+        pytest.skip("missing %s" % path)
+    g = np.load(path)
+    idx = np.concatenate([np.flatnonzero(g["has_ld"])[: count - 1], np.flatnonzero(~g["has_ld"])[:1]])
+    ref = np.where(g["has_ld"][idx], g["amp2_ld"][idx], g["amp2_d"][idx])
+    return g["momenta"][idx], g["weight"][idx], ref
 
 
 @pytest.mark.parametrize("name", workloads.ORDER)
@@ -75,13 +87,11 @@ if HEAVY:
 def test_amp2_matches_oracle_on_config_events(hg, name, precision, algo):
     n = workloads.CONFIGS[name]["n"]
     N = SMALL[name]
-    mom, w = oracle_events(name, N)
-    if n >= 7:
-        # keep the expensive oracle on events that bind: all cut-passing ones of a larger draw
-        big, wb = oracle_events(name, 200)
-        idx = np.concatenate([np.flatnonzero(wb != 0)[: N - 1], np.flatnonzero(wb == 0)[:1]])
-        mom, w = big[idx], wb[idx]
-    ref = oracle_amp2_cached(name, mom, extended=(n <= 7 or HEAVY))
+    if n >= 6:
+        mom, w, ref = golden_events(name, N)
+    else:
+        mom, w = oracle_events(name, N)
+        ref = oracle_amp2_cached(name, mom, extended=True)
     got = gpu_amp2(hg, mom, precision, algo)
     assert got.shape == ref.shape and np.all(np.isfinite(got)) and np.all(got > 0)
     rel = np.abs(got / ref - 1.0)
