@@ -17,17 +17,18 @@
 #include "amp2_chain.cuh"
 
 #ifndef HEGET_MINB32
-#define HEGET_MINB32 1      // fp32, n >= 6: __launch_bounds__ min CTAs of 256 threads per SM (2 caps at 128 registers)
+#define HEGET_MINB32 1      // fp32, n >= 6: __launch_bounds__ min CTAs of 256 threads per SM; 1 = no register cap (the six
+                            // unrolled levels take 250 registers; capped at 128 they spill 600 B: 8 gamma 132 against 102 ms)
 #endif
 #ifndef HEGET_MINW64
-#define HEGET_MINW64 8      // fp64, n >= 6: minimum resident warps per SM the register cap is set for; 8 = no cap
-                            // (the five unrolled levels need 220-250 registers; capped kernels spill)
+#define HEGET_MINW64 12     // fp64, n = 6: minimum resident warps per SM the register cap is set for (168 registers, no
+                            // spills; measured 8 -> 12: 24.0 -> 21.6 ms); n >= 7 run uncapped (six unrolled levels)
 #endif
 #ifndef HEGET_MINW64_N5
 #define HEGET_MINW64_N5 24  // ... of the 5-photon fp64 kernel (80 registers, no spills)
 #endif
 #ifndef HEGET_MINW32_N5
-#define HEGET_MINW32_N5 8   // ... of the 5-photon fp32 kernel; 8 = no cap
+#define HEGET_MINW32_N5 16  // ... of the 5-photon fp32 kernel (128 registers; measured 8 -> 16: 2.61 -> 2.24 ms)
 #endif
 
 // CTA size.  Small CTAs (64 threads: 2 events at n = 5) put more CTAs, each in its own phase
@@ -42,20 +43,31 @@ using TreeGeometry = Geometry<N, HEGET_TREE_CTA_THREADS>;
 namespace {
 
 #ifndef HEGET_CHAIN_KB32
-#define HEGET_CHAIN_KB32 5   // unrolled bottom levels of the factorised walk, fp32 / fp64
+#define HEGET_CHAIN_KB32 6   // unrolled bottom levels of the factorised walk, fp32 / fp64.  With nodes as cheap as the rho
+                             // table makes them, the per-lane address lists set up at the top of the unrolled part
+                             // must be amortised over many nodes: measured 5 (128 registers, 2 CTAs per SM) -> 6
+                             // (250 registers, 1 CTA): 6 gamma 14.8 -> 12.2 ms, 7 gamma 41.9 -> 29.4, 8 gamma 167 -> 102
 #endif
 #ifndef HEGET_CHAIN_KB64
-#define HEGET_CHAIN_KB64 5   // n >= 6, register cap lifted.  Round 1: five levels against four under a 128-register
-                             // cap: 6 gamma 34.1 -> 29.5 ms, 7 gamma 110.8 -> 96.6 ms, 8 gamma 440 -> 375 ms
+#define HEGET_CHAIN_KB64 6   // fp64, n >= 7 (n = 6: five levels, n = 5: four under its 80-register cap).  Six levels need the
+                             // E' entries of the list re-read from shared memory (kEByPtr) and still spill 0.7-1 KB at 255
+                             // registers, but win: measured 5 -> 6: 7 gamma 63.7 -> 56.8 ms, 8 gamma 257 -> 194 ms
+                             // (6 gamma 21.0 -> 23.8: stays at five)
 #endif
 template <int N, typename T>
 constexpr int kChainBottom = (sizeof(T) == 4) ? ((N < HEGET_CHAIN_KB32) ? N : HEGET_CHAIN_KB32)
-                                              : ((N < 6) ? 4 : HEGET_CHAIN_KB64);  // 5 gamma fp64: capped at 80 registers
+                                              : ((N < 6) ? 4 : ((N == 6) ? 5 : HEGET_CHAIN_KB64));
 
 // A CTA's batch lasts only a few microseconds at n = 5, so the DRAM latency of its momenta is a
 // visible fraction of it.  The fp32 kernel therefore sizes its grid to the number of resident CTAs
 // and loops over batches with the next batch's loads in flight (registers) while it computes the
 // current one (round 1: 6.48 -> 6.39 ms; the fp64 kernel is 1-6 % SLOWER that way).
+#ifndef HEGET_CHAIN_E_BY_PTR64
+#define HEGET_CHAIN_E_BY_PTR64 1   // fp64, six unrolled levels: re-read the E' entries of the list from shared memory
+#endif
+template <int N, typename T>
+constexpr bool kEByPtr = (sizeof(T) == 8) && (HEGET_CHAIN_E_BY_PTR64 != 0) && (kChainBottom<N, T> >= 6);
+
 #ifndef HEGET_PERSIST32
 #define HEGET_PERSIST32 1
 #endif
@@ -66,14 +78,14 @@ constexpr bool kPersistent = (HEGET_PERSIST32 != 0) && (sizeof(T) == 4) && (N ==
 template <int N, typename T>
 struct ChainTables {
     static constexpr int NW = 4 * (N * (N - 1) / 2);          // pair closing rows W
-    static constexpr int NK = (N * (N - 1) / 2) * N * 8;      // closing dots K
+    static constexpr int NK = kChainEntries<N>;               // closing dots K
     static constexpr int NR = kRhoEntries<N>;                 // rho of the last attachment
     static constexpr size_t BYTES = (size_t)TreeGeometry<N>::EPB * (NK + NR) * sizeof(Cx<T>);
 };
 
 template <int N, typename T>
 constexpr int kMinBlocks = ((sizeof(T) == 4) ? ((N == 5) ? HEGET_MINW32_N5 * 32 : HEGET_MINB32 * 256)
-                                             : ((N == 5) ? HEGET_MINW64_N5 : HEGET_MINW64) * 32) / TreeGeometry<N>::THREADS;
+                                             : ((N == 5) ? HEGET_MINW64_N5 : ((N == 6) ? HEGET_MINW64 : 8)) * 32) / TreeGeometry<N>::THREADS;
 
 template <int N, typename T>
 __global__ void __launch_bounds__(TreeGeometry<N>::THREADS, kMinBlocks<N, T>)
@@ -116,7 +128,7 @@ amp2_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_
         // first photon); ampsum = A(root)
         T ar = 0, ai = 0;
         const Spinor<T> f0 = {(T)1, (T)0, (T)0, (T)0};
-        WalkChain<N, 0, kChainBottom<N, T>, T>::run(s_P + ev_local * G::L, s_E + ev_local * 2 * N, hel, 0u, f0, ar, ai,
+        WalkChain<N, 0, kChainBottom<N, T>, T, kEByPtr<N, T>>::run(s_P + ev_local * G::L, s_E + ev_local * 2 * N, hel, 0u, f0, ar, ai,
                                                      s_K + ev_local * Tab::NK, s_R + ev_local * Tab::NR);
 
         // a8: |ampsum|^2 summed over the event's 2^N lanes, constant factors, store

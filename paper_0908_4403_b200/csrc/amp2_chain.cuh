@@ -14,8 +14,11 @@
 // by the depth-first walk and all n! orderings are visited; no ordering-summed quantity is
 // tabulated beyond the pair closing table W of v8 (amp2_common.cuh).  A node of n-2 photons closes
 // its two remaining orderings with W_ab . psi = z (W_ab . v): the dot product depends on the event
-// only, so it is tabulated per event (build_chain_table),
-//     K[(pair(a,b) N + j) 8 + 4 h_j + 2 h_a + h_b] = W_ab(h_a,h_b) . v(all \ {a,b}, j, h_j),
+// only, so it is tabulated per event (build_chain_table), indexed by the triple T = {j, a, b} of the
+// photons not in the node's parent, x < y < z, their helicities and which of them is j,
+//     K[(rank(T) 3 + slot(j)) 8 + 4 h_x + 2 h_y + h_z] = W_ab(h_a,h_b) . v(all \ {a,b}, j, h_j),
+// so that the three entries a node of n-3 photons needs (j = x, y, z) sit at ONE lane-dependent address
+// plus constants, and the 8 helicity combinations a warp reads at once are adjacent (one wavefront),
 // and the closing is z' K: 4 instructions instead of 8.  The walk does not carry z down: z is a
 // common factor of everything below a node, so each node RETURNS the sum of its subtree without it,
 //     A(node of n-2 photons) = K,   A(node) = sum over children j of rho_j A(child j),   ampsum = A(root)
@@ -31,11 +34,10 @@
 // at n = 8.  Nothing summed over orderings is tabulated: R and K are per-node factors, every ordered
 // prefix of up to n-2 photons is still one term of the walk.
 #pragma once
+#include <type_traits>
+
 #include "amp2_common.cuh"
 
-#ifndef HEGET_CHAIN_LEAN_MAXN
-#define HEGET_CHAIN_LEAN_MAXN 6   // build_chain_table: one work item per (pair, j, h_j) up to this N
-#endif
 
 template <typename T>
 struct alignas(2 * sizeof(T)) Cx {
@@ -84,57 +86,66 @@ __device__ __forceinline__ Cx<double> lds_cx(unsigned addr, double)
     asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(c.r), "=d"(c.i) : "r"(addr));
     return c;
 }
+// the three K entries of one node: the same lane-dependent address plus 0, 8 and 16 entries
+__device__ __forceinline__ void lds_cx3(unsigned addr, Cx<float>& a, Cx<float>& b, Cx<float>& c)
+{
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(a.r), "=f"(a.i) : "r"(addr));
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2+64];" : "=f"(b.r), "=f"(b.i) : "r"(addr));
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2+128];" : "=f"(c.r), "=f"(c.i) : "r"(addr));
+}
+__device__ __forceinline__ void lds_cx3(unsigned addr, Cx<double>& a, Cx<double>& b, Cx<double>& c)
+{
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(a.r), "=d"(a.i) : "r"(addr));
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2+128];" : "=d"(b.r), "=d"(b.i) : "r"(addr));
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2+256];" : "=d"(c.r), "=d"(c.i) : "r"(addr));
+}
 
-// Reads s_P, s_E and the pair closing table s_W (barrier before), ends with a barrier.
+// K table entries per event: [triple T (colex rank)][slot of j in T][4 h_x + 2 h_y + h_z]
+template <int N>
+constexpr int kChainEntries = (N * (N - 1) * (N - 2) / 6) * 24;
+
+// unrank a photon triple x < y < z from its colex rank tr = C(z,3) + C(y,2) + x
+__device__ __forceinline__ void unrank_triple(unsigned tr, unsigned& x, unsigned& y, unsigned& z)
+{
+    z = 2;
+    while ((z + 1) * z * (z - 1) / 6 <= tr) ++z;
+    const unsigned rem = tr - z * (z - 1) * (z - 2) / 6;
+    y = 1;
+    while ((y + 1) * y / 2 <= rem) ++y;
+    x = rem - y * (y - 1) / 2;
+}
+
+// Reads s_P, s_E and the pair closing table s_W (barrier before), ends with a barrier.  One work item
+// per (T, j in T, h_j): the vector v(all \ {a,b}, j, h_j) once, then its dot products with the four W
+// rows of the pair {a, b} = T \ j.
 template <int N, typename T, typename G = Geometry<N>>
 __device__ __forceinline__ void build_chain_table(const PEntry<T>* s_P, const EEntry<T>* s_E, const Spinor<T>* s_W,
                                                   Cx<T>* s_K)
 {
-    constexpr unsigned NP = N * (N - 1) / 2, ENTRIES = NP * N * 8u;
-    // one work item per (pair, j not in the pair, h_j): the vector v once, then its dot products with
-    // the four W entries of the pair (the K entries with j in {a, b} are holes and stay unwritten)
-    constexpr unsigned ITEMS = NP * (N - 2) * 2u;
+    constexpr unsigned NT = N * (N - 1) * (N - 2) / 6, ITEMS = NT * 6u;
     const int ev_local = threadIdx.x / G::L;
     const unsigned lane = threadIdx.x % G::L;
     const PEntry<T>* P = s_P + ev_local * G::L;
     const EEntry<T>* E = s_E + ev_local * 2 * N;
-    const Spinor<T>* W = s_W + ev_local * 4 * NP;
-    Cx<T>* K = s_K + ev_local * ENTRIES;
-    if constexpr (N <= HEGET_CHAIN_LEAN_MAXN) {
-        for (unsigned q = lane; q < ITEMS; q += G::L) {
-            const unsigned hj = q & 1u, t = q >> 1, jr = t % (N - 2), pair = t / (N - 2);
-            unsigned b = 1;
-            while ((b + 1) * b / 2 <= pair) ++b;
-            const unsigned a = pair - b * (b - 1) / 2;
-            unsigned j = jr;   // the jr-th photon outside {a, b}, a < b
-            if (j >= a) ++j;
-            if (j >= b) ++j;
-            const Spinor<T> v = chain_vector(P[(G::L - 1) ^ (1u << a) ^ (1u << b)], E[2 * j + hj]);
-    #pragma unroll
-            for (unsigned h = 0; h < 4; ++h) {
-                const Spinor<T> w = W[4 * pair + h];
-                Cx<T> k;
-                k.r = fma(w.r0, v.r0, fma(-w.i0, v.i0, fma(w.r1, v.r1, -(w.i1 * v.i1))));
-                k.i = fma(w.r0, v.i0, fma(w.i0, v.r0, fma(w.r1, v.i1, w.i1 * v.r1)));
-                K[(pair * N + j) * 8u + 4u * hj + h] = k;
-            }
-        }
-    } else {
-        // one entry per work item (the holes skipped).  From 7 photons on the table is < 1 % of the
-        // kernel either way, and ptxas allocates the unrolled tree below better after this form
-        // (8 gamma fp32: 223 ms against 232 ms with the loop above)
-        for (unsigned q = lane; q < ENTRIES; q += G::L) {
-            const unsigned h = q & 7u, pj = q >> 3, j = pj % N, pair = pj / N;
-            unsigned b = 1;
-            while ((b + 1) * b / 2 <= pair) ++b;
-            const unsigned a = pair - b * (b - 1) / 2;
-            if (j == a || j == b) continue;
-            const Spinor<T> v = chain_vector(P[(G::L - 1) ^ (1u << a) ^ (1u << b)], E[2 * j + (h >> 2)]);
-            const Spinor<T> w = W[4 * pair + (h & 3u)];
+    const Spinor<T>* W = s_W + ev_local * 4 * (N * (N - 1) / 2);
+    Cx<T>* K = s_K + ev_local * kChainEntries<N>;
+    for (unsigned q = lane; q < ITEMS; q += G::L) {
+        const unsigned hj = q & 1u, t = q >> 1, slot = t % 3u, tr = t / 3u;
+        unsigned x, y, z;
+        unrank_triple(tr, x, y, z);
+        const unsigned j = slot == 0 ? x : (slot == 1 ? y : z);
+        const unsigned a = slot == 0 ? y : x, b = slot == 2 ? y : z;   // a < b: the pair that closes
+        const Spinor<T> v = chain_vector(P[(G::L - 1) ^ (1u << a) ^ (1u << b)], E[2 * j + hj]);
+        const unsigned pair = b * (b - 1) / 2 + a;
+        // bit weight of h_j, h_a, h_b in 4 h_x + 2 h_y + h_z
+        const unsigned wj = 4u >> slot, wa = slot == 0 ? 2u : 4u, wb = slot == 2 ? 2u : 1u;
+#pragma unroll
+        for (unsigned h = 0; h < 4; ++h) {   // h = 2 h_a + h_b
+            const Spinor<T> w = W[4 * pair + h];
             Cx<T> k;
             k.r = fma(w.r0, v.r0, fma(-w.i0, v.i0, fma(w.r1, v.r1, -(w.i1 * v.i1))));
             k.i = fma(w.r0, v.i0, fma(w.i0, v.r0, fma(w.r1, v.i1, w.i1 * v.r1)));
-            K[q] = k;
+            K[(tr * 3u + slot) * 8u + wj * hj + wa * (h >> 1) + wb * (h & 1u)] = k;
         }
     }
     __syncthreads();
@@ -157,12 +168,8 @@ __device__ __forceinline__ void build_rho_table(const PEntry<T>* s_P, const EEnt
     Cx<T>* R = s_R + ev_local * kRhoEntries<N>;
     for (unsigned q = lane; q < ITEMS; q += G::L) {
         const unsigned hi = q & 1u, t = q >> 1, islot = t % (N - 3), tr = t / (N - 3);
-        // unrank the triple x < y < z: tr = C(z,3) + C(y,2) + x
-        unsigned z = 2;
-        while ((z + 1) * z * (z - 1) / 6 <= tr) ++z;
-        unsigned rem = tr - z * (z - 1) * (z - 2) / 6, y = 1;
-        while ((y + 1) * y / 2 <= rem) ++y;
-        const unsigned x = rem - y * (y - 1) / 2;
+        unsigned x, y, z;
+        unrank_triple(tr, x, y, z);
         unsigned i = islot;   // the islot-th photon outside {x, y, z}
         if (i >= x) ++i;
         if (i >= y) ++i;
@@ -186,18 +193,26 @@ __device__ __forceinline__ void build_rho_table(const PEntry<T>* s_P, const EEnt
 // of the remaining photons in the list of KB photons the unrolled part started from, kp[] = this
 // lane's K-table base of each position pair p < q (at q(q-1)/2 + p), jo[] = offset of (j, h_j)
 // for each position.  Ends at K = 3: the children are the nodes of n-2 photons, closed with K.
-template <int K, int KB, typename T>
+// EA = EEntry<T> (the list's E' entries held in registers) or unsigned (their 32-bit shared-memory address;
+// a and b are re-read where they are used: 4 T registers less per remaining photon, which is what lets six
+// levels nearly fit in fp64)
+template <typename T> __device__ __forceinline__ Cx<T> chain_ea(const EEntry<T>& e) { return {e.ar, e.ai}; }
+template <typename T> __device__ __forceinline__ Cx<T> chain_eb(const EEntry<T>& e) { return {e.br, e.bi}; }
+template <typename T> __device__ __forceinline__ Cx<T> chain_ea(unsigned e) { return lds_cx(e, T()); }
+template <typename T> __device__ __forceinline__ Cx<T> chain_eb(unsigned e) { return lds_cx(e + (unsigned)sizeof(Cx<T>), T()); }
+
+template <int K, int KB, typename T, typename EA = EEntry<T>>
 struct ChainBottom {
-    static constexpr int KP = KB * (KB - 1) / 2, KT = KB * (KB - 1) * (KB - 2) / 6;
-    // All table addresses are 32-bit shared-memory BYTE addresses / offsets:
-    // kp[] = this lane's K-table base of each position pair, jo[] = offset of (j, h_j) per position;
-    // rp[] = rho-table base of each position triple p < q < r (at C(r,3) + C(q,2) + p), io[] = offset of
-    // (i, h_i) in a triple's block per position (photon id x 12 + h_i x 6 entries; the members of T below
-    // i are subtracted at compile time), hb[] = this lane's helicity bit per position x one entry
+    static constexpr int KT = KB * (KB - 1) * (KB - 2) / 6;
+    // All table addresses are 32-bit shared-memory BYTE addresses / offsets, per position triple p < q < r
+    // of the list (at C(r,3) + C(q,2) + p): kt[] = address of this lane's three K entries (the lane's
+    // helicities of the triple folded in), rp[] = rho-table base of the triple; io[] = offset of (i, h_i) in
+    // a triple's rho block per position (photon id x 12 + h_i x 6 entries; the members of T below i are
+    // subtracted at compile time), hb[] = this lane's helicity bit per position x one entry
     static __device__ __forceinline__ void run(const PEntry<T>* __restrict__ PS, const int (&bit)[K],
-                                               const EEntry<T> (&e)[K], const int (&idx)[K],
-                                               const unsigned (&kp)[KP], const unsigned (&rp)[KT],
-                                               const unsigned (&jo)[KB], const unsigned (&io)[KB], const unsigned (&hb)[KB],
+                                               const EA (&e)[K], const int (&idx)[K],
+                                               const unsigned (&kt)[KT], const unsigned (&rp)[KT],
+                                               const unsigned (&io)[KB], const unsigned (&hb)[KB],
                                                const Spinor<T>& v, T& ar, T& ai)
     {
         static_assert(K >= 4, "a node of n-4 photons attaches i; the tables close the three levels below it");
@@ -205,24 +220,31 @@ struct ChainBottom {
 #pragma unroll
         for (int i = 0; i < K; ++i) {
             T rr, ri;
-            chain_rho(v, e[i], rr, ri);
+            EEntry<T> ei;
+            {
+                const Cx<T> b = chain_eb<T>(e[i]);
+                ei.br = b.r;
+                ei.bi = b.i;
+            }
+            chain_rho(v, ei, rr, ri);
             T cr = 0, ci = 0;
             if constexpr (K == 4) {
                 // the child holds n-3 photons; T = the other three positions p < q < r
                 const int p = idx[i == 0 ? 1 : 0], q = idx[i <= 1 ? 2 : 1], r = idx[i == 3 ? 2 : 3];
                 const int below = (p < idx[i]) + (q < idx[i]) + (r < idx[i]);
                 constexpr unsigned EB = sizeof(Cx<T>);
-                const unsigned R = rp[r * (r - 1) * (r - 2) / 6 + q * (q - 1) / 2 + p] + io[idx[i]] - 12 * EB * below;
+                const int t = r * (r - 1) * (r - 2) / 6 + q * (q - 1) / 2 + p;
+                const unsigned R = rp[t] + io[idx[i]] - 12 * EB * below;
                 const Cx<T> r0 = lds_cx(R + hb[p], T()), r1 = lds_cx(R + hb[q] + 2 * EB, T()),
                             r2 = lds_cx(R + hb[r] + 4 * EB, T());
-                const Cx<T> k0 = lds_cx(kp[r * (r - 1) / 2 + q] + jo[p], T()), k1 = lds_cx(kp[r * (r - 1) / 2 + p] + jo[q], T()),
-                            k2 = lds_cx(kp[q * (q - 1) / 2 + p] + jo[r], T());
+                Cx<T> k0, k1, k2;
+                lds_cx3(kt[t], k0, k1, k2);
                 chain_acc(r0.r, r0.i, k0.r, k0.i, cr, ci);
                 chain_acc(r1.r, r1.i, k1.r, k1.i, cr, ci);
                 chain_acc(r2.r, r2.i, k2.r, k2.i, cr, ci);
             } else {
                 int sub_bit[K - 1];
-                EEntry<T> sub_e[K - 1];
+                EA sub_e[K - 1];
                 int sub_idx[K - 1];
 #pragma unroll
                 for (int m = 0; m < K - 1; ++m) {
@@ -231,8 +253,13 @@ struct ChainBottom {
                     sub_idx[m] = idx[m + (m >= i ? 1 : 0)];
                 }
                 const PEntry<T>* Pn = PS + bit[i];
-                const Spinor<T> vc = chain_vector(*Pn, e[i]);
-                ChainBottom<K - 1, KB, T>::run(Pn, sub_bit, sub_e, sub_idx, kp, rp, jo, io, hb, vc, cr, ci);
+                {
+                    const Cx<T> a = chain_ea<T>(e[i]);
+                    ei.ar = a.r;
+                    ei.ai = a.i;
+                }
+                const Spinor<T> vc = chain_vector(*Pn, ei);
+                ChainBottom<K - 1, KB, T, EA>::run(Pn, sub_bit, sub_e, sub_idx, kt, rp, io, hb, vc, cr, ci);
             }
             chain_acc(rr, ri, cr, ci, sr, si);
         }
@@ -244,7 +271,7 @@ struct ChainBottom {
 // Depth-first walk of the upper levels (`used` = photons already attached, uniform over the CTA;
 // returns A(node) in ar, ai);
 // when KB photons remain the unrolled ChainBottom<KB> takes over.  Needs N - KB >= 0 and KB >= 4.
-template <int N, int DEPTH, int KB, typename T>
+template <int N, int DEPTH, int KB, typename T, bool E_BY_PTR = false>
 struct WalkChain {
     static __device__ __forceinline__ void run(const PEntry<T>* __restrict__ P, const EEntry<T>* __restrict__ E,
                                                unsigned hel, unsigned used, const Spinor<T>& v, T& ar, T& ai,
@@ -252,34 +279,29 @@ struct WalkChain {
     {
         unsigned avail = ((1u << N) - 1u) & ~used;
         if constexpr (N - DEPTH == KB) {
-            constexpr int KP = KB * (KB - 1) / 2, KT = KB * (KB - 1) * (KB - 2) / 6;
+            constexpr int KT = KB * (KB - 1) * (KB - 2) / 6;
             constexpr unsigned EB = sizeof(Cx<T>);
             int bit[KB], idx[KB], photon[KB];
-            unsigned jo[KB], io[KB], hb[KB], hbit[KB];
-            EEntry<T> e[KB];
+            unsigned io[KB], hb[KB], hbit[KB];
+            using EA = std::conditional_t<E_BY_PTR, unsigned, EEntry<T>>;
+            EA e[KB];
 #pragma unroll
             for (int m = 0; m < KB; ++m) {
                 const int i = __ffs(avail) - 1;
                 avail &= avail - 1u;
                 bit[m] = 1 << i;
                 hbit[m] = (hel >> i) & 1u;
-                e[m] = E[2 * i + hbit[m]];
+                if constexpr (E_BY_PTR)
+                    e[m] = (unsigned)__cvta_generic_to_shared(&E[2 * i + hbit[m]]);
+                else
+                    e[m] = E[2 * i + hbit[m]];
                 idx[m] = m;
                 photon[m] = i;
                 hb[m] = EB * hbit[m];
-                jo[m] = EB * (8 * i + 4 * hbit[m]);
                 io[m] = EB * (12 * i + 6 * hbit[m]);
             }
             const unsigned k_base = (unsigned)__cvta_generic_to_shared(Kt), r_base = (unsigned)__cvta_generic_to_shared(Rt);
-            unsigned kp[KP];
-#pragma unroll
-            for (int q = 1; q < KB; ++q)
-#pragma unroll
-                for (int p = 0; p < q; ++p) {  // photon[] is increasing
-                    const int pair = photon[q] * (photon[q] - 1) / 2 + photon[p];
-                    kp[q * (q - 1) / 2 + p] = k_base + EB * (pair * (N * 8) + 2 * hbit[p] + hbit[q]);
-                }
-            unsigned rp[KT];
+            unsigned rp[KT], kt[KT];
 #pragma unroll
             for (int r = 2; r < KB; ++r)
 #pragma unroll
@@ -288,8 +310,10 @@ struct WalkChain {
                     for (int p = 0; p < q; ++p) {  // colex rank of the photon triple
                         const int tr = photon[r] * (photon[r] - 1) * (photon[r] - 2) / 6 + photon[q] * (photon[q] - 1) / 2 + photon[p];
                         rp[r * (r - 1) * (r - 2) / 6 + q * (q - 1) / 2 + p] = r_base + EB * (tr * (12 * (N - 3)));
+                        kt[r * (r - 1) * (r - 2) / 6 + q * (q - 1) / 2 + p] =
+                            k_base + EB * (tr * 24 + 4 * hbit[p] + 2 * hbit[q] + hbit[r]);
                     }
-            ChainBottom<KB, KB, T>::run(P + used, bit, e, idx, kp, rp, jo, io, hb, v, ar, ai);
+            ChainBottom<KB, KB, T, EA>::run(P + used, bit, e, idx, kt, rp, io, hb, v, ar, ai);
         } else {
             T sr = 0, si = 0;
             while (avail) {
@@ -300,7 +324,7 @@ struct WalkChain {
                 T rr, ri, cr, ci;
                 chain_rho(v, e, rr, ri);
                 const Spinor<T> vc = chain_vector(P[S], e);
-                WalkChain<N, DEPTH + 1, KB, T>::run(P, E, hel, S, vc, cr, ci, Kt, Rt);
+                WalkChain<N, DEPTH + 1, KB, T, E_BY_PTR>::run(P, E, hel, S, vc, cr, ci, Kt, Rt);
                 chain_acc(rr, ri, cr, ci, sr, si);
             }
             ar = sr;

@@ -106,9 +106,8 @@ __device__ __forceinline__ void build_tables(double g, const double* s_mom, PEnt
     __syncthreads();
 }
 
-// Closing table: U[2 b + h] = <vbar| E'_b(h) P_{all \ b} = (a pp + q, a qbar + pm), one row vector per
-// photon and helicity (amp2_tree.cuh, close_weyl).  Reads s_P and s_E (barrier before), ends with
-// a barrier.
+// Closing row U_b(h) = <vbar| E'_b(h) P_{all \ b} = (a pp + q, a qbar + pm), one row vector per photon
+// and helicity (amp2_tree.cuh, close_weyl).
 template <typename T>
 __device__ __forceinline__ Spinor<T> closing_entry(const EEntry<T>& e, const PEntry<T>& p)
 {
@@ -120,23 +119,11 @@ __device__ __forceinline__ Spinor<T> closing_entry(const EEntry<T>& e, const PEn
     return u;
 }
 
-template <int N, typename T, typename G = Geometry<N>>
-__device__ __forceinline__ void build_closing_table(const PEntry<T>* s_P, const EEntry<T>* s_E, Spinor<T>* s_U)
-{
-    const int ev_local = threadIdx.x / G::L;
-    const unsigned lane = threadIdx.x % G::L;
-    for (unsigned q = lane; q < 2u * N; q += G::L)
-        s_U[ev_local * 2 * N + q] = closing_entry(s_E[ev_local * 2 * N + q],
-                                                  s_P[ev_local * G::L + ((G::L - 1) ^ (1u << (q >> 1)))]);
-    __syncthreads();
-}
-
 // Pair closing table: the two orderings that share a prefix of n-2 photons end with (a, b) or
 // (b, a), and both close on the same spinor psi of that prefix:
 //   <vbar|E'_b P_{all\b} E'_a psi + <vbar|E'_a P_{all\a} E'_b psi = (U_b E'_a + U_a E'_b) . psi = W_ab . psi,
 // one row vector per unordered pair a < b and per helicity of a and b,
 //   W[4 (b(b-1)/2 + a) + 2 h_a + h_b],   (u0, u1) E' = (-u0 + a u1, -b u0 + u1).
-// Reads s_U and s_E (barrier before), ends with a barrier.
 template <typename T>
 __device__ __forceinline__ void accumulate_row_times_vertex(const Spinor<T>& u, const EEntry<T>& e, Spinor<T>& r)
 {
@@ -146,31 +133,8 @@ __device__ __forceinline__ void accumulate_row_times_vertex(const Spinor<T>& u, 
     r.i1 += fma(-e.br, u.i0, fma(-e.bi, u.r0, u.i1));
 }
 
-template <int N, typename T, typename G = Geometry<N>>
-__device__ __forceinline__ void build_pair_table(const Spinor<T>* s_U, const EEntry<T>* s_E, Spinor<T>* s_W)
-{
-    constexpr unsigned ITEMS = 4u * (N * (N - 1) / 2);
-    const int ev_local = threadIdx.x / G::L;
-    const unsigned lane = threadIdx.x % G::L;
-    const Spinor<T>* U = s_U + ev_local * 2 * N;
-    const EEntry<T>* E = s_E + ev_local * 2 * N;
-    for (unsigned q = lane; q < ITEMS; q += G::L) {
-        const unsigned pair = q >> 2, ha = (q >> 1) & 1u, hb = q & 1u;
-        unsigned b = 1;
-        while ((b + 1) * b / 2 <= pair) ++b;
-        const unsigned a = pair - b * (b - 1) / 2;
-        Spinor<T> w = {(T)0, (T)0, (T)0, (T)0};
-        accumulate_row_times_vertex(U[2 * b + hb], E[2 * a + ha], w);
-        accumulate_row_times_vertex(U[2 * a + ha], E[2 * b + hb], w);
-        s_W[ev_local * ITEMS + q] = w;
-    }
-    __syncthreads();
-}
-
-// The same table straight from the P and E tables (the closing entries U_a, U_b of an item are
-// evaluated in place, bit-identical to the two-step form): one phase and one barrier less, which
-// is what counts in the latency-bound small-n kernels.  SYNC = false leaves the barrier to the
-// caller (amp2.cu fills the shared first two tree levels in the same phase).
+// Built straight from the P and E tables (the closing rows U_a, U_b of an item are evaluated in place).
+// Reads s_P and s_E (barrier before); ends with a barrier unless SYNC = false.
 template <int N, typename T, typename G = Geometry<N>, bool SYNC = true>
 __device__ __forceinline__ void build_pair_table_direct(const PEntry<T>* s_P, const EEntry<T>* s_E, Spinor<T>* s_W)
 {
