@@ -52,9 +52,10 @@ def model_flops_per_event(n):
 def executed_flops_per_event(n, precision="fp32"):
     """What the tree kernels execute per event, tables excluded.
     n >= 5 (lane per helicity assignment, factorised nodes psi = z v, csrc/amp2_chain.cuh): 2^n lanes;
-    every ordered prefix of up to n-3 photons is rho (4 FMA) + the vector v of the node (5 FMA + 1 MUL)
-    + the accumulation rho A (4 FMA) = 27 flop; a prefix of n-2 photons (its two remaining orderings
-    closed by the per-event table of closing dots) is rho + accumulation = 16 flop.
+    every ordered prefix of up to n-4 photons is rho (4 FMA) + the vector v of the node (5 FMA + 1 MUL)
+    + the accumulation rho A (4 FMA) = 27 flop; a prefix of n-3 photons needs no vector (the rho of its
+    three children come from the per-event rho table, their closing dots from the K table): rho +
+    accumulation + three complex FMAs R K = 20 FMA = 40 flop.
     n <= 4 (thread per event, csrc/amp2_thread.cu): nodes are shared between helicity assignments (a
     prefix is evaluated once per helicity assignment of ITS photons): n = 4: 8 vectors v1 (11 flop),
     24 vectors v2 (11), 48 rho (8), 48 scalings/accumulations of psi_2 (16), 96 closing dots (16);
@@ -62,8 +63,8 @@ def executed_flops_per_event(n, precision="fp32"):
     The kernels' whole count, tables included, is read from the SASS (sass_flops_per_event) or from the
     ncu summaries under profiles/."""
     if n >= 5:
-        upper = sum(math.factorial(n) // math.factorial(n - l) for l in range(1, n - 2))
-        return 2 ** n * (27 * upper + 16 * (math.factorial(n) // 2))
+        upper = sum(math.factorial(n) // math.factorial(n - l) for l in range(1, n - 3))
+        return 2 ** n * (27 * upper + 40 * (math.factorial(n) // 6))
     if n == 4:
         return 8 * 11 + 24 * 11 + 48 * 8 + 48 * 16 + 96 * 16
     if n == 3:
@@ -115,7 +116,8 @@ def sass_flops_per_event(n, precision):
     from paper_0908_4403_b200 import binding
     val = None
     try:
-        out = subprocess.run(["cuobjdump", "-sass", binding.LIB_PATH], capture_output=True, text=True, timeout=120).stdout
+        tool = "/usr/local/cuda/bin/cuobjdump" if os.path.exists("/usr/local/cuda/bin/cuobjdump") else "cuobjdump"
+        out = subprocess.run([tool, "-sass", binding.LIB_PATH], capture_output=True, text=True, timeout=300).stdout
         want = "amp2_thread_kernelILi%dE%s" % (n, "d" if precision == "fp64" else "f")
         body, on = [], False
         for line in out.splitlines():
@@ -123,9 +125,20 @@ def sass_flops_per_event(n, precision):
                 on = want in line
             elif on:
                 body.append(line)
-        ops = [m.group(1) for m in (re.match(r"\s+/\*[0-9a-f]{4,}\*/\s+(?:@!?U?P\d\s+)?([A-Z0-9_.]+)", l) for l in body) if m]
-        if ops and not any(o.startswith("BRA") for o in ops[:-2]):
-            count = lambda p: sum(1 for o in ops if o.split(".")[0] == p)
+        ops, straight = [], True
+        for l in body:
+            m = re.match(r"\s+/\*([0-9a-f]{4,})\*/\s+(@!?U?P\d\s+)?([A-Z0-9_.]+)(.*?);", l)
+            if not m:
+                continue
+            addr, pred, op, rest = int(m.group(1), 16), m.group(2), m.group(3), m.group(4)
+            if op == "EXIT" and not pred:
+                break                              # the slow paths of division and square root and the padding follow
+            if op.startswith("BRA"):
+                t = re.search(r"0x([0-9a-f]+)", rest)
+                straight = straight and bool(t) and int(t.group(1), 16) > addr   # forward only (skips a slow-path call)
+            ops.append(op.split(".")[0])
+        if ops and straight:
+            count = lambda p: sum(1 for o in ops if o == p)
             val = float(2 * (count("DFMA") + count("FFMA")) + count("DMUL") + count("FMUL") + count("DADD") + count("FADD"))
     except Exception:
         val = None
@@ -559,6 +572,31 @@ def main():
                         row.update({"frac_of_measured_peak": model * nn / (ms * 1e-3) / pkk["measured"], "note": note})
                     table.append(row)
         result["per_config"] = table
+
+        # 2 photons are HBM- and launch-latency bound (136 B and ~340 flop per event): the same kernel on 2^20
+        # events against the measured HBM copy rate, beside config 1's 65,536 events (a few microseconds,
+        # i.e. the launch-latency floor)
+        hbm = _hbm_peak()
+        c2 = workloads.CONFIGS["2gamma"]
+        rows2 = []
+        for n2 in (c2["N"], 1 << 20, 1 << 23):
+            m2, _ = hg.gen_events(c2["seed"], 2, n2, mode=c2["mode"], a=c2["a"])
+            o2 = torch.empty(n2, dtype=torch.float64, device=hg.device)
+            for _ in range(3):
+                hg.amp2(m2, FP64, out=o2)
+            ts = []
+            for _ in range(7):
+                flush_buf.zero_()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                hg.amp2(m2, FP64, out=o2)
+                e1.record()
+                torch.cuda.synchronize()
+                ts.append(e0.elapsed_time(e1))
+            ms2 = sorted(ts)[len(ts) // 2]
+            rows2.append({"events": n2, "amp2_ms": ms2, "events_per_s": n2 / (ms2 * 1e-3),
+                          "hbm_gbs": n2 * 136 / (ms2 * 1e-3) / 1e9, "frac_of_hbm_peak": n2 * 136 / (ms2 * 1e-3) / 1e9 / hbm["value"]})
+        result["two_photon_hbm"] = {"bytes_per_event": 136, "hbm_peak_gbs": hbm, "precision": "fp64", "rows": rows2}
         result["peaks_tflops"] = {p: {k: v / 1e12 for k, v in d.items()} for p, d in peaks.items()}
         result["hbm_peak_gbs"] = _hbm_peak()
 
