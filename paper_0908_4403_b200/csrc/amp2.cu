@@ -54,9 +54,12 @@ namespace {
                              // registers, but win: measured 5 -> 6: 7 gamma 63.7 -> 56.8 ms, 8 gamma 257 -> 194 ms
                              // (6 gamma 21.0 -> 23.8: stays at five)
 #endif
+#ifndef HEGET_CHAIN_KB64_N5
+#define HEGET_CHAIN_KB64_N5 4
+#endif
 template <int N, typename T>
 constexpr int kChainBottom = (sizeof(T) == 4) ? ((N < HEGET_CHAIN_KB32) ? N : HEGET_CHAIN_KB32)
-                                              : ((N < 6) ? 4 : ((N == 6) ? 5 : HEGET_CHAIN_KB64));
+                                              : ((N < 6) ? HEGET_CHAIN_KB64_N5 : ((N == 6) ? 5 : HEGET_CHAIN_KB64));
 
 // A CTA's batch lasts only a few microseconds at n = 5, so the DRAM latency of its momenta is a
 // visible fraction of it.  The fp32 kernel therefore sizes its grid to the number of resident CTAs
