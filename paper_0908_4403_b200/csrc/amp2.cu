@@ -146,8 +146,9 @@ cudaError_t launch_one(const heget_ctx* ctx, const double* momenta, double* out,
 {
     using G = TreeGeometry<N>;
     constexpr size_t dyn = ChainTables<N, T>::BYTES;
-    // more than the 48 KB a kernel gets without asking (n = 8); set once per kernel
-    static const cudaError_t attr =
+    // more than the 48 KB a kernel gets without asking (n = 8).  Set on every launch: the attribute belongs to the
+    // current device, and a process may hold contexts on several
+    const cudaError_t attr =
         cudaFuncSetAttribute(amp2_kernel<N, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
     if (attr != cudaSuccess) return attr;
     const int64_t n_batches = (n_events + G::EPB - 1) / G::EPB;

@@ -54,3 +54,34 @@ def test_flop_models_match_the_node_counts_of_the_survey():
     assert abs(bench.model_flops_per_event(2) / 1.09e3 - 1) < 0.01
     assert abs(bench.model_flops_per_event(4) / 7.5e4 - 1) < 0.01
     assert abs(bench.model_flops_per_event(8) / 2.06e9 - 1) < 0.01
+
+
+import pytest
+
+
+@pytest.mark.gpu
+def test_headline_line_carries_the_contract_and_a_fresh_ncu_summary():
+    """python bench.py (headline config, no sweep): the JSON line has every key the driver's contract names,
+    the roofline numerator comes from a committed ncu summary of THE kernel that ran (status ok: same kernel,
+    same event count, duration within 5 % of the one measured in this run), and its DRAM traffic is the
+    algorithmic traffic, not more."""
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--steps", "5", "--warmup", "3", "--no-sweep",
+                          "--no-cpu-baseline"], capture_output=True, text=True, timeout=900)
+    assert out.returncode == 0, out.stderr[-2000:]
+    line = json.loads(out.stdout.strip().splitlines()[-1])
+    for key in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+                "vs_baseline", "dtype", "data", "config", "clocks", "e2e", "pipeline", "gpu_launches", "roofline"):
+        assert key in line, key
+    assert line["config"]["workload"] == "4gamma" and line["dtype"] == "f64" and line["vs_baseline"] is None
+    assert line["gpu_launches"] == 3 * 5 and line["value"] > 1e9
+    assert line["e2e"]["h2d_bytes_per_step"] == (1 << 20) * (6 * 32 + 8) and 0 < line["e2e"]["value"] < line["value"]
+    assert 0 < line["pipeline"]["value"] < line["value"]
+    r = line["roofline"]
+    assert r["bound"] == "alu" and r["kernel"].startswith("amp2_thread_kernel<4,double>")
+    assert r["ncu_summary"]["status"] == "ok", r["ncu_summary"]
+    assert abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12 and 0.3 < r["frac"] < 1.0
+    assert 0.9 < r["traffic"] / r["algorithmic_bytes"] < 1.1
+    # the SASS count of the loaded library and the ncu-counted figure describe the same straight-line kernel
+    sys.path.insert(0, ROOT)
+    import bench
+    assert abs(bench.sass_flops_per_event(4, "fp64") / r["flops_per_event"] - 1.0) < 0.01

@@ -194,3 +194,28 @@ def test_invalid_arguments_return_einval(hg):
     assert lib.heget_amp2_algo(ctx, buf.data_ptr(), 4, FP64, ALGO_SUBSET, out.data_ptr(), 4, None) == 0
     assert lib.heget_xsec_reduce(ctx, out.data_ptr(), out.data_ptr(), 4, 4, None, None) == -1
     assert b"invalid" in lib.heget_strerror(-1)
+
+
+@pytest.mark.parametrize("n", [3, 4, 5])
+def test_forward_photon_stress_set_near_the_eta_cut(hg, n):
+    """The events that decide the 1e-12 gate (hard part 2): cut-passing events whose most
+    forward photon sits just inside |eta| < 2.5 and whose beams are strongly boosted, where t_S = (p1 - K_S)^2
+    cancels by up to 10^4.  Selected from 3 x 10^5 events of the oracle's generator (y up to 2.5, beyond the
+    configs' 1.5), compared one by one with oracle<long double> in all three organisations of the sum."""
+    mom, w = oracle.gen_events(77, n, 300000, mode=oracle.MODE_LOGUNIFORM, a=100.0 * n, b=2000.0 * n, y_max=2.5,
+                               apply_cuts=True)
+    k = mom[:, 2:]
+    pt = np.hypot(k[:, :, 1], k[:, :, 2])
+    eta = np.arcsinh(k[:, :, 3] / pt)
+    sel = np.flatnonzero((w != 0) & (np.abs(eta).max(axis=1) > 2.45))
+    count = {3: 400, 4: 400, 5: 120}[n]
+    assert sel.size >= count
+    sel = sel[:count]
+    ref = oracle.amp2(mom[sel], extended=True)
+    for algo in ALGOS:
+        got = gpu_amp2(hg, mom[sel], FP64, algo)
+        rel = np.abs(got / ref - 1.0)
+        report("stress n=%d fp64 %s" % (n, ALGO_NAME[algo]), rel, np.ones(len(rel), bool))
+        assert np.all(rel <= TOL64)
+    got32 = gpu_amp2(hg, mom[sel], FP32, ALGO_TREE)
+    assert np.all(np.abs(got32 / ref - 1.0) <= TOL32)
