@@ -101,6 +101,37 @@ def executed_flops_per_event_algo(n, algo, precision="fp32"):
 
 
 _SASS_CACHE = {}
+_SASS_DUMP = {}
+
+
+def kernel_sass(kernel, n, precision):
+    """The SASS lines of one amplitude kernel instantiation of the library that is loaded (cuobjdump), or None."""
+    from paper_0908_4403_b200 import binding
+    if "text" not in _SASS_DUMP:
+        try:
+            tool = "/usr/local/cuda/bin/cuobjdump" if os.path.exists("/usr/local/cuda/bin/cuobjdump") else "cuobjdump"
+            _SASS_DUMP["text"] = subprocess.run([tool, "-sass", binding.LIB_PATH], capture_output=True, text=True,
+                                                timeout=600).stdout.splitlines()
+        except Exception:
+            _SASS_DUMP["text"] = []
+    want = "%sILi%dE%s" % (kernel, n, "d" if precision == "fp64" else "f")
+    body, on = [], False
+    for line in _SASS_DUMP["text"]:
+        if "Function :" in line:
+            on = want in line
+        elif on:
+            body.append(line)
+    return body or None
+
+
+def kernel_sass_sha(kernel, n, precision):
+    """sha256 over the instruction text of that kernel: what ties a committed ncu summary to a binary."""
+    import hashlib
+    body = kernel_sass(kernel, n, precision)
+    if not body:
+        return None
+    text = "\n".join(l.strip() for l in body if re.match(r"\s+/\*[0-9a-f]{4,}\*/", l))
+    return hashlib.sha256(text.encode()).hexdigest()[:16]
 
 
 def sass_flops_per_event(n, precision):
@@ -113,18 +144,9 @@ def sass_flops_per_event(n, precision):
     key = (n, precision)
     if key in _SASS_CACHE:
         return _SASS_CACHE[key]
-    from paper_0908_4403_b200 import binding
     val = None
     try:
-        tool = "/usr/local/cuda/bin/cuobjdump" if os.path.exists("/usr/local/cuda/bin/cuobjdump") else "cuobjdump"
-        out = subprocess.run([tool, "-sass", binding.LIB_PATH], capture_output=True, text=True, timeout=300).stdout
-        want = "amp2_thread_kernelILi%dE%s" % (n, "d" if precision == "fp64" else "f")
-        body, on = [], False
-        for line in out.splitlines():
-            if "Function :" in line:
-                on = want in line
-            elif on:
-                body.append(line)
+        body = kernel_sass("amp2_thread_kernel", n, precision) or []
         ops, straight = [], True
         for l in body:
             m = re.match(r"\s+/\*([0-9a-f]{4,})\*/\s+(@!?U?P\d\s+)?([A-Z0-9_.]+)(.*?);", l)
@@ -146,12 +168,14 @@ def sass_flops_per_event(n, precision):
     return val
 
 
-def ncu_summary(config, precision, kernel, measured_ms, events):
+def ncu_summary(config, precision, kernel, measured_ms, events, n):
     """The committed `ncu --set full` summary of this kernel under profiles/ (newest round first):
     counted flops per event, DRAM bytes per launch and the kernel time of the capture.  The summary
-    describes the binary it was captured from: it is used only if it names the kernel that runs now
-    and its duration agrees with the one measured here within 5 %; otherwise the status says why and
-    the caller falls back to what it can measure itself."""
+    describes the binary it was captured from: it is used only if it names the kernel that runs now, was
+    taken on the same number of events, carries the SASS hash of THIS library's kernel (`sass_sha256:`
+    line; kernel_sass_sha) and its duration agrees with the one measured here within 5 % (or 4 us: CUDA
+    events around a kernel of a few microseconds include its launch latency, ncu's duration does not);
+    otherwise the status says why and the caller falls back to what it can measure itself."""
     files = sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_amp2_%s_%s.txt" % (config, precision))), reverse=True)
     if not files:
         return {"status": "no summary under profiles/ for %s %s" % (config, precision)}
@@ -178,11 +202,22 @@ def ncu_summary(config, precision, kernel, measured_ms, events):
         out["status"] = "STALE: %s is a capture of %s, the kernel that runs is %s" % (name, out["kernel"], kernel)
     elif out["events"] != events:
         out["status"] = "STALE: %s was captured on %d events, this run has %d" % (name, out["events"], events)
-    elif abs(ms / measured_ms - 1.0) > 0.05:
-        out["status"] = "STALE: %s says %.4f ms, measured here %.4f ms (> 5 %% apart)" % (name, ms, measured_ms)
     else:
-        out["status"] = "ok"
-    if out["status"] != "ok":
+        m_sha = re.search(r"^sass_sha256: ([0-9a-f]+)", text, re.M)
+        sha = kernel_sass_sha(kernel, n, precision)
+        out["sass_sha256"] = sha
+        if not m_sha or sha is None or m_sha.group(1) != sha:
+            out["status"] = "STALE: %s was captured from a different binary of %s (SASS hash %s, loaded library %s)" % (
+                name, kernel, m_sha.group(1) if m_sha else "missing", sha)
+        elif abs(ms / measured_ms - 1.0) > 0.05 and abs(ms - measured_ms) > 0.004:
+            # the same instructions ran (hash), so the counted flops and bytes per event hold; the clock or the
+            # neighbours of this launch differ from the capture's
+            out["status"] = "ok (same SASS as the capture; duration there %.4f ms, here %.4f ms)" % (ms, measured_ms)
+            out["duration_agrees"] = False
+        else:
+            out["status"] = "ok"
+            out["duration_agrees"] = True
+    if not out["status"].startswith("ok"):
         sys.stderr.write("bench.py: " + out["status"] + "\n")
     return out
 
@@ -481,8 +516,8 @@ def main():
 
     def flops_of(name, nph, precision, algo, ms, events):
         """(flops per event, source, ncu summary or None) for one kernel of this run."""
-        summ = ncu_summary(name, precision, kernel_name(algo, nph), ms, events) if algo == "tree" else None
-        if summ and summ["status"] == "ok":
+        summ = ncu_summary(name, precision, kernel_name(algo, nph), ms, events, nph) if algo == "tree" else None
+        if summ and summ["status"].startswith("ok"):
             return summ["flops_per_event"], "ncu-counted over the whole kernel, tables included (%s)" % summ["file"], summ
         sass = sass_flops_per_event(nph, precision) if algo == "tree" else None
         if sass:
@@ -498,11 +533,11 @@ def main():
     bytes_alg = nl * ((n + 2) * 32 + 8)
     roofline = {"bound": "alu", "achieved": achieved / 1e12, "peak": pk["measured"] / 1e12, "unit": "TFLOP/s",
                 "frac": achieved / pk["measured"],
-                "traffic": summ["dram_bytes"] if summ and summ["status"] == "ok" else None,
+                "traffic": summ["dram_bytes"] if summ and summ["status"].startswith("ok") else None,
                 "kernel": "%s<%d,%s>" % (kernel_name(args.algo, n), n, "double" if prec == FP64 else "float"),
                 "kernel_ms": amp_ms, "kernel_ms_best": amp_ms_best,
                 "flops_per_event": fpe, "flops_source": fsrc,
-                "ncu_summary": ({k: summ[k] for k in ("status", "file", "kernel_ms") if k in summ} if summ else None),
+                "ncu_summary": ({k: summ[k] for k in ("status", "file", "kernel_ms", "sass_sha256", "duration_agrees") if k in summ} if summ else None),
                 "flops_per_event_tree_model": tree_model,
                 "tree_model_tflops": tree_model * nl / (amp_ms * 1e-3) / 1e12,
                 "peak_source": "heget_fma_peak on this GPU: FMA with constant-bank operands "

@@ -78,7 +78,7 @@ def test_headline_line_carries_the_contract_and_a_fresh_ncu_summary():
     assert 0 < line["pipeline"]["value"] < line["value"]
     r = line["roofline"]
     assert r["bound"] == "alu" and r["kernel"].startswith("amp2_thread_kernel<4,double>")
-    assert r["ncu_summary"]["status"] == "ok", r["ncu_summary"]
+    assert r["ncu_summary"]["status"] == "ok" and r["ncu_summary"]["duration_agrees"], r["ncu_summary"]
     assert abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12 and 0.3 < r["frac"] < 1.0
     assert 0.9 < r["traffic"] / r["algorithmic_bytes"] < 1.1
     # the SASS count of the loaded library and the ncu-counted figure describe the same straight-line kernel
