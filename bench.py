@@ -30,12 +30,12 @@ if ROOT not in sys.path:
 METRIC = "events/s of summed |M|^2 for u ubar->n gamma"
 UNIT = "events/s"
 ALGOS = {"tree": 0, "subset": 1, "two-sided": 2}
-THREAD_MAXN = 4     # n <= 4: one thread per event (csrc/amp2_thread.cu); n >= 5: one lane per helicity assignment
+THREAD_MAXN = 5     # n <= 5: one thread per event (csrc/amp2_thread.cu); n >= 6: one lane per helicity assignment
 
 
 def kernel_name(algo, n):
     if algo == "tree":
-        return "amp2_thread_kernel" if n <= THREAD_MAXN else "amp2_kernel"
+        return "amp2_kernel" if n > THREAD_MAXN else ("amp2_thread5_kernel" if n == 5 else "amp2_thread_kernel")
     return {"subset": "amp2_subset_kernel", "two-sided": "amp2_twosided_kernel"}[algo]
 
 
@@ -51,20 +51,24 @@ def model_flops_per_event(n):
 
 def executed_flops_per_event(n, precision="fp32"):
     """What the tree kernels execute per event, tables excluded.
-    n >= 5 (lane per helicity assignment, factorised nodes psi = z v, csrc/amp2_chain.cuh): 2^n lanes;
+    n >= 6 (lane per helicity assignment, factorised nodes psi = z v, csrc/amp2_chain.cuh): 2^n lanes;
     every ordered prefix of up to n-4 photons is rho (4 FMA) + the vector v of the node (5 FMA + 1 MUL)
     + the accumulation rho A (4 FMA) = 27 flop; a prefix of n-3 photons needs no vector (the rho of its
     three children come from the per-event rho table, their closing dots from the K table): rho +
     accumulation + three complex FMAs R K = 20 FMA = 40 flop.
-    n <= 4 (thread per event, csrc/amp2_thread.cu): nodes are shared between helicity assignments (a
-    prefix is evaluated once per helicity assignment of ITS photons): n = 4: 8 vectors v1 (11 flop),
+    n <= 5 (thread per event, csrc/amp2_thread.cu): nodes are shared between helicity assignments (a
+    prefix is evaluated once per helicity assignment of ITS photons): n = 5: per photon triple 12 vectors
+    v2 and 6 v3 (11 flop), 48 rho (8), 24 products rho rho and 24 accumulations of Psi (16 each), 4 pair
+    rows (32) and 32 closing dots (16 + 2), plus 10 v1 and 10 U (11); n = 4: 8 vectors v1 (11 flop),
     24 vectors v2 (11), 48 rho (8), 48 scalings/accumulations of psi_2 (16), 96 closing dots (16);
     n = 3: 6 vectors (11), 24 dots (16 + 2); n = 2: the closing rows only (counted with the tables).
     The kernels' whole count, tables included, is read from the SASS (sass_flops_per_event) or from the
     ncu summaries under profiles/."""
-    if n >= 5:
+    if n >= 6:
         upper = sum(math.factorial(n) // math.factorial(n - l) for l in range(1, n - 3))
         return 2 ** n * (27 * upper + 40 * (math.factorial(n) // 6))
+    if n == 5:
+        return 10 * (18 * 11 + 48 * 8 + 48 * 16 + 4 * 32 + 32 * 18) + 20 * 11
     if n == 4:
         return 8 * 11 + 24 * 11 + 48 * 8 + 48 * 16 + 96 * 16
     if n == 3:
@@ -114,7 +118,8 @@ def kernel_sass(kernel, n, precision):
                                                 timeout=600).stdout.splitlines()
         except Exception:
             _SASS_DUMP["text"] = []
-    want = "%sILi%dE%s" % (kernel, n, "d" if precision == "fp64" else "f")
+    t = "d" if precision == "fp64" else "f"
+    want = "%sI%sE" % (kernel, t) if kernel == "amp2_thread5_kernel" else "%sILi%dE%s" % (kernel, n, t)
     body, on = [], False
     for line in _SASS_DUMP["text"]:
         if "Function :" in line:
@@ -146,8 +151,8 @@ def sass_flops_per_event(n, precision):
         return _SASS_CACHE[key]
     val = None
     try:
-        body = kernel_sass("amp2_thread_kernel", n, precision) or []
-        ops, straight = [], True
+        body = kernel_sass(kernel_name("tree", n), n, precision) or []
+        ops, loops, ok = [], [], True            # ops: (address, mnemonic); loops: (target, address of the backward branch)
         for l in body:
             m = re.match(r"\s+/\*([0-9a-f]{4,})\*/\s+(@!?U?P\d\s+)?([A-Z0-9_.]+)(.*?);", l)
             if not m:
@@ -157,11 +162,16 @@ def sass_flops_per_event(n, precision):
                 break                              # the slow paths of division and square root and the padding follow
             if op.startswith("BRA"):
                 t = re.search(r"0x([0-9a-f]+)", rest)
-                straight = straight and bool(t) and int(t.group(1), 16) > addr   # forward only (skips a slow-path call)
-            ops.append(op.split(".")[0])
-        if ops and straight:
-            count = lambda p: sum(1 for o in ops if o == p)
-            val = float(2 * (count("DFMA") + count("FFMA")) + count("DMUL") + count("FMUL") + count("DADD") + count("FADD"))
+                ok = ok and bool(t)
+                if t and int(t.group(1), 16) <= addr:
+                    loops.append((int(t.group(1), 16), addr))     # forward branches only skip a slow-path call
+            ops.append((addr, op.split(".")[0]))
+        # n <= 4: no loop at all; n = 5: exactly one, the rolled loop over the 10 photon triples
+        trips = {5: 10}.get(n, 0)
+        if ops and ok and len(loops) == (1 if trips else 0):
+            w = {"DFMA": 2, "FFMA": 2, "DMUL": 1, "FMUL": 1, "DADD": 1, "FADD": 1}
+            inside = lambda a: bool(loops) and loops[0][0] <= a <= loops[0][1]
+            val = float(sum(w.get(o, 0) * (trips if inside(a) else 1) for a, o in ops))
     except Exception:
         val = None
     _SASS_CACHE[key] = val

@@ -1,8 +1,8 @@
 // amp2.cu -- heget_amp2: summed squared helicity amplitude of u ubar -> n gamma (product code).
 //
-// n <= 4 runs one thread per event (amp2_thread.cu).  This file is the kernel for n >= 5:
-// one lane per photon-helicity configuration (2^N lanes per event), CTAs of max(64, 2^N) threads
-// holding 64/2^N events (two at n = 5, one from n = 6 on).  All lanes of a CTA walk the SAME
+// n <= 5 runs one thread per event (amp2_thread.cu).  This file is the kernel for n >= 6:
+// one lane per photon-helicity configuration (2^N lanes per event), one event per CTA of 2^N
+// threads.  All lanes of a CTA walk the SAME
 // permutation tree in lockstep (no divergence); they differ only in which helicity entry of the
 // per-photon and per-subset tables they read.  Per event the CTA first builds, in shared memory,
 //   - the E table (vxxxx0 for both helicities of every photon),
@@ -24,16 +24,8 @@
 #define HEGET_MINW64 12     // fp64, n = 6: minimum resident warps per SM the register cap is set for (168 registers, no
                             // spills; measured 8 -> 12: 24.0 -> 21.6 ms); n >= 7 run uncapped (six unrolled levels)
 #endif
-#ifndef HEGET_MINW64_N5
-#define HEGET_MINW64_N5 24  // ... of the 5-photon fp64 kernel (80 registers, no spills)
-#endif
-#ifndef HEGET_MINW32_N5
-#define HEGET_MINW32_N5 16  // ... of the 5-photon fp32 kernel (128 registers; measured 8 -> 16: 2.61 -> 2.24 ms)
-#endif
 
-// CTA size.  Small CTAs (64 threads: 2 events at n = 5) put more CTAs, each in its own phase
-// (load / tables / tree), on an SM at the same number of warps, which overlaps the latency-bound
-// phases better (measured on B200 in round 1: 1-2 % at 5-7 photons, 10 % at 4).
+// CTA size: at least 64 threads; from 6 photons on an event's 2^N lanes are one CTA.
 #ifndef HEGET_TREE_CTA_THREADS
 #define HEGET_TREE_CTA_THREADS 64
 #endif
@@ -49,33 +41,19 @@ namespace {
                              // (250 registers, 1 CTA): 6 gamma 14.8 -> 12.2 ms, 7 gamma 41.9 -> 29.4, 8 gamma 167 -> 102
 #endif
 #ifndef HEGET_CHAIN_KB64
-#define HEGET_CHAIN_KB64 6   // fp64, n >= 7 (n = 6: five levels, n = 5: four under its 80-register cap).  Six levels need the
+#define HEGET_CHAIN_KB64 6   // fp64, n >= 7 (n = 6: five levels).  Six levels need the
                              // E' entries of the list re-read from shared memory (kEByPtr) and still spill 0.7-1 KB at 255
                              // registers, but win: measured 5 -> 6: 7 gamma 63.7 -> 56.8 ms, 8 gamma 257 -> 194 ms
                              // (6 gamma 21.0 -> 23.8: stays at five)
 #endif
-#ifndef HEGET_CHAIN_KB64_N5
-#define HEGET_CHAIN_KB64_N5 4
-#endif
 template <int N, typename T>
-constexpr int kChainBottom = (sizeof(T) == 4) ? ((N < HEGET_CHAIN_KB32) ? N : HEGET_CHAIN_KB32)
-                                              : ((N < 6) ? HEGET_CHAIN_KB64_N5 : ((N == 6) ? 5 : HEGET_CHAIN_KB64));
+constexpr int kChainBottom = (sizeof(T) == 4) ? HEGET_CHAIN_KB32 : ((N == 6) ? 5 : HEGET_CHAIN_KB64);
 
-// A CTA's batch lasts only a few microseconds at n = 5, so the DRAM latency of its momenta is a
-// visible fraction of it.  The fp32 kernel therefore sizes its grid to the number of resident CTAs
-// and loops over batches with the next batch's loads in flight (registers) while it computes the
-// current one (round 1: 6.48 -> 6.39 ms; the fp64 kernel is 1-6 % SLOWER that way).
 #ifndef HEGET_CHAIN_E_BY_PTR64
 #define HEGET_CHAIN_E_BY_PTR64 1   // fp64, six unrolled levels: re-read the E' entries of the list from shared memory
 #endif
 template <int N, typename T>
 constexpr bool kEByPtr = (sizeof(T) == 8) && (HEGET_CHAIN_E_BY_PTR64 != 0) && (kChainBottom<N, T> >= 6);
-
-#ifndef HEGET_PERSIST32
-#define HEGET_PERSIST32 1
-#endif
-template <int N, typename T>
-constexpr bool kPersistent = (HEGET_PERSIST32 != 0) && (sizeof(T) == 4) && (N == 5);
 
 // per-event entries of the tables of the factorised walk (dynamic shared memory of amp2_kernel)
 template <int N, typename T>
@@ -87,13 +65,11 @@ struct ChainTables {
 };
 
 template <int N, typename T>
-constexpr int kMinBlocks = ((sizeof(T) == 4) ? ((N == 5) ? HEGET_MINW32_N5 * 32 : HEGET_MINB32 * 256)
-                                             : ((N == 5) ? HEGET_MINW64_N5 : ((N == 6) ? HEGET_MINW64 : 8)) * 32) / TreeGeometry<N>::THREADS;
+constexpr int kMinBlocks = ((sizeof(T) == 4) ? HEGET_MINB32 * 256 : ((N == 6) ? HEGET_MINW64 : 8) * 32) / TreeGeometry<N>::THREADS;
 
 template <int N, typename T>
 __global__ void __launch_bounds__(TreeGeometry<N>::THREADS, kMinBlocks<N, T>)
-amp2_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_t n_events, double g,
-            int64_t n_batches)
+amp2_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_t n_events, double g)
 {
     using G = TreeGeometry<N>;
     using Tile = MomentaTile<N, G>;
@@ -113,31 +89,25 @@ amp2_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_
     const int ev_local = threadIdx.x / G::L;
     const unsigned hel = threadIdx.x % G::L;
 
+    const int64_t ev0 = (int64_t)blockIdx.x * G::EPB;
     double2 pf[Tile::PF];
-    int64_t batch = blockIdx.x;
-    Tile::load(momenta, batch * G::EPB, n_events, pf);                       // a1
-    do {  // one pass unless kPersistent (grid = number of batches)
-        Tile::store(s_mom, pf);
-        __syncthreads();
-        if constexpr (kPersistent<N, T>) {
-            if (batch + gridDim.x < n_batches) Tile::load(momenta, (batch + gridDim.x) * G::EPB, n_events, pf);
-        }
-        build_tables<N, T, G>(g, s_mom, s_P, s_E, s_s2);                        // a4, a5 (every build_* ends with a barrier)
-        build_pair_table_direct<N, T, G>(s_P, s_E, s_W);
-        build_chain_table<N, T, G>(s_P, s_E, s_W, s_K);
-        build_rho_table<N, T, G>(s_P, s_E, s_R);
+    Tile::load(momenta, ev0, n_events, pf);                                  // a1
+    Tile::store(s_mom, pf);
+    __syncthreads();
+    build_tables<N, T, G>(g, s_mom, s_P, s_E, s_s2);                            // a4, a5 (every build_* ends with a barrier)
+    build_pair_table_direct<N, T, G>(s_P, s_E, s_W);
+    build_chain_table<N, T, G>(s_P, s_E, s_W, s_K);
+    build_rho_table<N, T, G>(s_P, s_E, s_R);
 
-        // a2, a6, a7: psi_0 = u(p1,+)/sqrt(2E1) = (1,0) is the root vector (rho = v_0 + b v_1 = 1 for every
-        // first photon); ampsum = A(root)
-        T ar = 0, ai = 0;
-        const Spinor<T> f0 = {(T)1, (T)0, (T)0, (T)0};
-        WalkChain<N, 0, kChainBottom<N, T>, T, kEByPtr<N, T>>::run(s_P + ev_local * G::L, s_E + ev_local * 2 * N, hel, 0u, f0, ar, ai,
-                                                     s_K + ev_local * Tab::NK, s_R + ev_local * Tab::NR);
+    // a2, a6, a7: psi_0 = u(p1,+)/sqrt(2E1) = (1,0) is the root vector (rho = v_0 + b v_1 = 1 for every
+    // first photon); ampsum = A(root)
+    T ar = 0, ai = 0;
+    const Spinor<T> f0 = {(T)1, (T)0, (T)0, (T)0};
+    WalkChain<N, 0, kChainBottom<N, T>, T, kEByPtr<N, T>>::run(s_P + ev_local * G::L, s_E + ev_local * 2 * N, hel, 0u, f0, ar, ai,
+                                                 s_K + ev_local * Tab::NK, s_R + ev_local * Tab::NR);
 
-        // a8: |ampsum|^2 summed over the event's 2^N lanes, constant factors, store
-        finish_event<N, T, G>(ar, ai, s_mom, s_s2, s_red, g, out, batch * G::EPB, n_events);
-        if constexpr (kPersistent<N, T>) __syncthreads();                    // tables are rewritten next round
-    } while (kPersistent<N, T> && (batch += gridDim.x) < n_batches);
+    // a8: |ampsum|^2 summed over the event's 2^N lanes, constant factors, store
+    finish_event<N, T, G>(ar, ai, s_mom, s_s2, s_red, g, out, ev0, n_events);
 }
 
 template <int N, typename T>
@@ -151,16 +121,8 @@ cudaError_t launch_one(const heget_ctx* ctx, const double* momenta, double* out,
     const cudaError_t attr =
         cudaFuncSetAttribute(amp2_kernel<N, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
     if (attr != cudaSuccess) return attr;
-    const int64_t n_batches = (n_events + G::EPB - 1) / G::EPB;
-    int64_t blocks = n_batches;
-    if (kPersistent<N, T>) {
-        int per_sm = 0;
-        cudaError_t err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, amp2_kernel<N, T>, G::THREADS, dyn);
-        if (err != cudaSuccess) return err;
-        const int64_t resident = (int64_t)ctx->sm_count * (per_sm > 0 ? per_sm : 1);
-        if (blocks > resident) blocks = resident;
-    }
-    amp2_kernel<N, T><<<(unsigned)blocks, G::THREADS, dyn, stream>>>(momenta, out, n_events, g, n_batches);
+    const int64_t blocks = (n_events + G::EPB - 1) / G::EPB;
+    amp2_kernel<N, T><<<(unsigned)blocks, G::THREADS, dyn, stream>>>(momenta, out, n_events, g);
     return cudaGetLastError();
 }
 
@@ -169,7 +131,6 @@ cudaError_t launch_n(const heget_ctx* ctx, int n, const double* momenta, double*
                      cudaStream_t stream)
 {
     switch (n) {
-        case 5: return launch_one<5, T>(ctx, momenta, out, n_events, g, stream);
         case 6: return launch_one<6, T>(ctx, momenta, out, n_events, g, stream);
         case 7: return launch_one<7, T>(ctx, momenta, out, n_events, g, stream);
         case 8: return launch_one<8, T>(ctx, momenta, out, n_events, g, stream);
@@ -184,7 +145,7 @@ cudaError_t heget_launch_amp2(const heget_ctx* ctx, const double* momenta, int n
 {
     *launches = 0;
     if (N == 0) return cudaSuccess;
-    if (n <= 4) return heget_launch_amp2_thread(ctx, momenta, n, precision, out_amp2, N, stream, launches);
+    if (n <= 5) return heget_launch_amp2_thread(ctx, momenta, n, precision, out_amp2, N, stream, launches);
     *launches = 1;
     if (precision == HEGET_FP32) return launch_n<float>(ctx, n, momenta, out_amp2, N, ctx->g, stream);
     return launch_n<double>(ctx, n, momenta, out_amp2, N, ctx->g, stream);

@@ -1,5 +1,5 @@
 // amp2_chain.cuh -- the permutation tree of eq. (6) with every off-shell spinor held
-// in factorised form (product code, v9; amp2.cu uses it for n >= 5).
+// in factorised form (product code, v9; amp2.cu uses it for n >= 6; amp2_thread.cu borrows its node helpers).
 //
 // For a massless photon of definite helicity the chiral block of eps-slash has rank one
 // (eps-slash^2 = eps.eps = 0): in the normalisation of amp2_tables.cuh, a b = 1 and

@@ -1,9 +1,10 @@
-// amp2_thread.cu -- heget_amp2 for n = 2, 3, 4: one THREAD per event (product code).
+// amp2_thread.cu -- heget_amp2 for n = 2 .. 5: one THREAD per event (product code).
 //
 // This is the paper's own mapping (one phase-space point per thread) applied to the
 // permutation tree of eq. (6) in the two-component, factorised form of amp2_tables.cuh
 // and amp2_chain.cuh.  For n <= 4 an event's whole tree, for ALL 2^n photon-helicity assignments, fits
-// one thread's registers (2^n complex accumulators) plus a few per-thread columns of shared memory,
+// one thread's registers (2^n complex accumulators) plus a few per-thread columns of shared memory
+// (n = 5, further down: the 32 accumulators live in the column too),
 // and the thread never idles: the lane-per-helicity kernel of amp2.cu spends most of a 4-photon event
 // in table phases that occupy 4, 6 or 14 of an event's 16 lanes and in the index arithmetic of its
 // work-item loops, which here is all folded at compile time.
@@ -404,6 +405,235 @@ amp2_thread_kernel(const double* __restrict__ momenta, double* __restrict__ out,
     if (live) out[ev] = norm * m2;
 }
 
+// ---- n = 5: one thread per event with the 32 accumulators in the thread's shared-memory column --------------
+//
+// Same mathematics; the unit of work is an unordered triple T3 = {i,j,k} of photons with the pair {a,b} left
+// over: Psi_T3(h_i,h_j,h_k) = sum over the 6 ordered prefixes (p,q,r) of T3 of rho(p->q) rho(q->r) v(T3, r, h_r)
+// (each ordered prefix one node, evaluated once per helicity assignment of ITS photons), closed by the pair rows:
+// ampsum(h) += W_ab(h_a,h_b) . Psi_T3(h_i,h_j,h_k).  2^5 complex accumulators do not fit the register file
+// beside Psi, so they live in the column and are read-modified-written once per triple.
+#ifndef HEGET_THREAD5_CTA
+#define HEGET_THREAD5_CTA 32
+#endif
+#ifndef HEGET_THREAD5_MINB64
+#define HEGET_THREAD5_MINB64 4
+#endif
+#ifndef HEGET_THREAD5_MINB32
+#define HEGET_THREAD5_MINB32 8
+#endif
+constexpr int kCol5V1 = 0, kCol5U = 10, kCol5P2 = 20, kCol5P3 = 30, kCol5E = 40, kCol5Amp = 90;   // spinor slots; amp in Cx words
+constexpr int kColumnWords5 = 90 + 32;                                                              // Cx words per thread
+
+// the 10 units of work: triple {i < j < k} in colex order and the pair {a < b} left over
+struct Triple5 { unsigned char i, j, k, a, b; };
+__constant__ Triple5 c_triples5[10] = {{0, 1, 2, 3, 4}, {0, 1, 3, 2, 4}, {0, 2, 3, 1, 4}, {1, 2, 3, 0, 4}, {0, 1, 4, 2, 3},
+                                       {0, 2, 4, 1, 3}, {1, 2, 4, 0, 3}, {0, 3, 4, 1, 2}, {1, 3, 4, 0, 2}, {2, 3, 4, 0, 1}};
+
+// E' entry of photon `ph` and helicity h (compile-time) from the lambda = +1 entry kept in the column:
+// lambda = -1 is a' = -conj(b), b' = -conj(a) (amp2_tables.cuh)
+template <int CTA, int H, typename T>
+__device__ __forceinline__ EEntry<T> e5(const Cx<T>* col, int ph)
+{
+    const Cx<T> a = col[(2 * (kCol5E + ph)) * CTA], b = col[(2 * (kCol5E + ph) + 1) * CTA];
+    if constexpr (H == 1) return {a.r, a.i, b.r, b.i};
+    return {-b.r, b.i, -a.r, a.i};
+}
+
+template <int CTA, typename T>
+__device__ __forceinline__ void put5(Cx<T>* col, int w, T a, T b, T c, T d)
+{
+    col[(2 * w) * CTA] = {a, b};
+    col[(2 * w + 1) * CTA] = {c, d};
+}
+template <int CTA, typename T>
+__device__ __forceinline__ Spinor<T> get5(const Cx<T>* col, int w)
+{
+    const Cx<T> a = col[(2 * w) * CTA], b = col[(2 * w + 1) * CTA];
+    return {a.r, a.i, b.r, b.i};
+}
+template <int CTA, typename T>
+__device__ __forceinline__ PEntry<T> get5p(const Cx<T>* col, int w)
+{
+    const Cx<T> a = col[(2 * w) * CTA], b = col[(2 * w + 1) * CTA];
+    return {a.r, a.i, b.r, b.i};
+}
+
+template <typename T>
+__global__ void __launch_bounds__(HEGET_THREAD5_CTA, (sizeof(T) == 8) ? HEGET_THREAD5_MINB64 : HEGET_THREAD5_MINB32)
+amp2_thread5_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_t n_events, double g)
+{
+    constexpr int N = 5, CTA = HEGET_THREAD5_CTA;
+    constexpr unsigned ALL = 31u;
+    extern __shared__ __align__(16) unsigned char s_dyn5[];
+    Cx<T>* col = reinterpret_cast<Cx<T>*>(s_dyn5) + threadIdx.x;
+
+    int64_t ev = (int64_t)blockIdx.x * CTA + threadIdx.x;
+    const bool live = ev < n_events;
+    if (!live) ev = n_events - 1;
+
+    double e1, e2, k[N][4];
+    {
+        const double2* src = reinterpret_cast<const double2*>(momenta) + ev * (2 * (N + 2));
+        e1 = __ldg(src).x;
+        e2 = __ldg(src + 2).x;
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+            const double2 a = __ldg(src + 4 + 2 * i), b = __ldg(src + 5 + 2 * i);
+            k[i][0] = a.x; k[i][1] = a.y; k[i][2] = b.x; k[i][3] = b.y;
+        }
+    }
+    const double shat = 4.0 * e1 * e2;
+    const double scale = (sizeof(T) == 4) ? sqrt(shat) : 1.0;
+
+    EEntry<T> e[N][2];
+    double norm = 2.0 * g * g * shat;
+#pragma unroll
+    for (int i = 0; i < N; ++i) norm *= 0.5 * make_photon_entries<T>(k[i], &e[i][1], &e[i][0]);
+    if constexpr (sizeof(T) == 4) {
+        const double inv = 1.0 / shat;
+#pragma unroll
+        for (int i = 0; i < N - 1; ++i) norm *= inv;
+    }
+
+    {   // tables: v1[2 i + h], U[2 b + h], P_ij at j (j-1)/2 + i, P_ijk at the colex rank of the triple
+        Kinematics<N, sizeof(T) == 8> kin;
+        kin.init(k, e1, g, scale);
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+            const PEntry<T> p1 = kin.template subset<T>(1u << i);
+            const PEntry<T> p4 = kin.template subset<T>(ALL ^ (1u << i));
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const Spinor<T> v = chain_vector(p1, e[i][h]), u = closing_entry(e[i][h], p4);
+                put5<CTA>(col, kCol5V1 + 2 * i + h, v.r0, v.i0, v.r1, v.i1);
+                put5<CTA>(col, kCol5U + 2 * i + h, u.r0, u.i0, u.r1, u.i1);
+            }
+        }
+#pragma unroll
+        for (int j = 1; j < N; ++j)
+#pragma unroll
+            for (int i = 0; i < j; ++i) {
+                const PEntry<T> p = kin.template subset<T>((1u << i) | (1u << j));
+                put5<CTA>(col, kCol5P2 + j * (j - 1) / 2 + i, p.pp, p.pm, p.px, p.py);
+            }
+#pragma unroll
+        for (int kk = 2; kk < N; ++kk)
+#pragma unroll
+            for (int j = 1; j < kk; ++j)
+#pragma unroll
+                for (int i = 0; i < j; ++i) {
+                    const PEntry<T> p = kin.template subset<T>((1u << i) | (1u << j) | (1u << kk));
+                    put5<CTA>(col, kCol5P3 + kk * (kk - 1) * (kk - 2) / 6 + j * (j - 1) / 2 + i, p.pp, p.pm, p.px, p.py);
+                }
+#pragma unroll
+        for (int i = 0; i < N; ++i) put5<CTA>(col, kCol5E + i, e[i][1].ar, e[i][1].ai, e[i][1].br, e[i][1].bi);
+#pragma unroll
+        for (int h = 0; h < 32; ++h) col[(kCol5Amp + h) * CTA] = {(T)0, (T)0};
+    }
+    __syncwarp();   // keeps the compiler from forwarding the column through registers (it would spill)
+
+    // A rolled loop over the 10 triples (the photon indices are run-time values read from constant memory, the
+    // E' entries come from the column): fully unrolled, the kernel was 225 KB of straight-line code and its few
+    // warps per SM waited for instructions more than for anything else (ncu: no_instruction 3.4 per issue).
+#pragma unroll 1
+    for (int t = 0; t < 10; ++t) {
+        const int t3[3] = {c_triples5[t].i, c_triples5[t].j, c_triples5[t].k};
+        const int a = c_triples5[t].a, b = c_triples5[t].b;
+        const PEntry<T> p3 = get5p<CTA>(col, kCol5P3 + t);
+        Spinor<T> psi[8];   // index 4 h_i + 2 h_j + h_k
+#pragma unroll
+        for (int rr = 0; rr < 3; ++rr) {
+            // last photon r of the prefix; p < q the other two: orderings (p, q, r) and (q, p, r)
+            const int r = t3[2 - rr], p = t3[rr == 2 ? 1 : 0], q = t3[rr == 0 ? 1 : 2];
+            const int sr = rr, sp = (rr == 2) ? 1 : 2, sq = (rr == 0) ? 1 : 0;   // bit of h_r, h_p, h_q in psi's index
+            const PEntry<T> p2 = get5p<CTA>(col, kCol5P2 + q * (q - 1) / 2 + p);
+            const EEntry<T> ep[2] = {e5<CTA, 0>(col, p), e5<CTA, 1>(col, p)}, eq[2] = {e5<CTA, 0>(col, q), e5<CTA, 1>(col, q)},
+                            er[2] = {e5<CTA, 0>(col, r), e5<CTA, 1>(col, r)};
+            Cx<T> A[2][2], B[2][2], C[2][2], D[2][2];   // rho(p->q)[hp][hq], rho(q->r)[hq][hr], rho(q->p)[hq][hp], rho(p->r)[hp][hr]
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const Spinor<T> v1p = get5<CTA>(col, kCol5V1 + 2 * p + h), v1q = get5<CTA>(col, kCol5V1 + 2 * q + h);
+                const Spinor<T> v2q = chain_vector(p2, eq[h]), v2p = chain_vector(p2, ep[h]);   // last = q / p, helicity h
+#pragma unroll
+                for (int g2 = 0; g2 < 2; ++g2) {
+                    chain_rho(v1p, eq[g2], A[h][g2].r, A[h][g2].i);
+                    chain_rho(v1q, ep[g2], C[h][g2].r, C[h][g2].i);
+                    chain_rho(v2q, er[g2], B[h][g2].r, B[h][g2].i);
+                    chain_rho(v2p, er[g2], D[h][g2].r, D[h][g2].i);
+                }
+            }
+#pragma unroll
+            for (int hr = 0; hr < 2; ++hr) {
+                const Spinor<T> v3 = chain_vector(p3, er[hr]);
+#pragma unroll
+                for (int hp = 0; hp < 2; ++hp)
+#pragma unroll
+                    for (int hq = 0; hq < 2; ++hq) {
+                        Cx<T> z = cx_mul(A[hp][hq], B[hq][hr]);
+                        chain_acc(C[hq][hp].r, C[hq][hp].i, D[hp][hr].r, D[hp][hr].i, z.r, z.i);
+                        Spinor<T>& ps = psi[(hr << sr) | (hp << sp) | (hq << sq)];
+                        if (rr == 0) {
+                            ps.r0 = fma(z.r, v3.r0, -(z.i * v3.i0));
+                            ps.i0 = fma(z.r, v3.i0, z.i * v3.r0);
+                            ps.r1 = fma(z.r, v3.r1, -(z.i * v3.i1));
+                            ps.i1 = fma(z.r, v3.i1, z.i * v3.r1);
+                        } else {
+                            chain_acc(z.r, z.i, v3.r0, v3.i0, ps.r0, ps.i0);
+                            chain_acc(z.r, z.i, v3.r1, v3.i1, ps.r1, ps.i1);
+                        }
+                    }
+            }
+        }
+        const EEntry<T> ea[2] = {e5<CTA, 0>(col, a), e5<CTA, 1>(col, a)}, eb[2] = {e5<CTA, 0>(col, b), e5<CTA, 1>(col, b)};
+        // accumulator of assignment h sits at word h: bits of the triple's and the pair's photons, as byte offsets
+        Cx<T>* amp = col + kCol5Amp * CTA;
+#pragma unroll
+        for (int ha = 0; ha < 2; ++ha) {
+            const Spinor<T> ua = get5<CTA>(col, kCol5U + 2 * a + ha);
+#pragma unroll
+            for (int hb = 0; hb < 2; ++hb) {
+                const Spinor<T> w = pair_row(ua, get5<CTA>(col, kCol5U + 2 * b + hb), ea[ha], eb[hb]);
+                const int hab = (ha << a) | (hb << b);
+                // eight accumulators at a time: all loads, then all stores (the compiler must keep a load behind an
+                // earlier store it cannot tell apart, which would make the 32 updates of a triple one serial chain)
+                Cx<T> acc[8];
+#pragma unroll
+                for (int c = 0; c < 8; ++c)
+                    acc[c] = amp[((((c >> 2) & 1) << t3[0]) | (((c >> 1) & 1) << t3[1]) | ((c & 1) << t3[2]) | hab) * CTA];
+#pragma unroll
+                for (int c = 0; c < 8; ++c) {
+                    const Cx<T> dot = row_dot(w, psi[c]);
+                    acc[c].r += dot.r;
+                    acc[c].i += dot.i;
+                }
+#pragma unroll
+                for (int c = 0; c < 8; ++c)
+                    amp[((((c >> 2) & 1) << t3[0]) | (((c >> 1) & 1) << t3[1]) | ((c & 1) << t3[2]) | hab) * CTA] = acc[c];
+            }
+        }
+    }
+    __syncwarp();
+
+    double m2 = 0.0;
+#pragma unroll
+    for (int h = 0; h < 32; ++h) {
+        const Cx<T> acc = col[(kCol5Amp + h) * CTA];
+        m2 += (double)acc.r * (double)acc.r + (double)acc.i * (double)acc.i;
+    }
+    if (live) out[ev] = norm * m2;
+}
+
+template <typename T>
+cudaError_t launch_thread5(const double* momenta, double* out, int64_t n_events, double g, cudaStream_t stream)
+{
+    constexpr size_t dyn = sizeof(Cx<T>) * kColumnWords5 * HEGET_THREAD5_CTA;
+    const cudaError_t attr = cudaFuncSetAttribute(amp2_thread5_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
+    if (attr != cudaSuccess) return attr;
+    const int64_t blocks = (n_events + HEGET_THREAD5_CTA - 1) / HEGET_THREAD5_CTA;
+    amp2_thread5_kernel<T><<<(unsigned)blocks, HEGET_THREAD5_CTA, dyn, stream>>>(momenta, out, n_events, g);
+    return cudaGetLastError();
+}
+
 template <int N, typename T>
 cudaError_t launch_thread(const double* momenta, double* out, int64_t n_events, double g, cudaStream_t stream)
 {
@@ -428,6 +658,8 @@ cudaError_t heget_launch_amp2_thread(const heget_ctx* ctx, const double* momenta
                            : launch_thread<3, double>(momenta, out_amp2, N, ctx->g, stream);
         case 4: return f32 ? launch_thread<4, float>(momenta, out_amp2, N, ctx->g, stream)
                            : launch_thread<4, double>(momenta, out_amp2, N, ctx->g, stream);
+        case 5: return f32 ? launch_thread5<float>(momenta, out_amp2, N, ctx->g, stream)
+                           : launch_thread5<double>(momenta, out_amp2, N, ctx->g, stream);
         default: return cudaErrorInvalidValue;
     }
 }

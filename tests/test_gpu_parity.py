@@ -61,8 +61,8 @@ def report(tag, rel, passing):
           % (tag, rel.size, int(passing.sum()), p.max(), np.median(p), rel.max(), np.median(rel)))
 
 
-# sizes: several CTAs plus a ragged tail for every n (events per CTA: 64 for n <= 4, one thread per event;
-# 2 at n = 5 and 1 from n = 6 on, one lane per photon-helicity assignment)
+# sizes: several CTAs plus a ragged tail for every n (events per CTA: 64 for n <= 4 and 32 at n = 5, one thread
+# per event; 1 from n = 6 on, one lane per photon-helicity assignment)
 SMALL = {"2gamma": 64 * 5 + 3, "3gamma": 64 * 2 + 7, "4gamma": 16 * 9 + 5, "5gamma": 2 * 20 + 3, "6gamma": 4 * 6 + 1,
          "7gamma": 9, "8gamma": 5}
 GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
