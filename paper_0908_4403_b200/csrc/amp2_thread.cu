@@ -421,8 +421,43 @@ amp2_thread_kernel(const double* __restrict__ momenta, double* __restrict__ out,
 #ifndef HEGET_THREAD5_MINB32
 #define HEGET_THREAD5_MINB32 8
 #endif
-constexpr int kCol5V1 = 0, kCol5U = 10, kCol5P2 = 20, kCol5P3 = 30, kCol5E = 40, kCol5Amp = 90;   // spinor slots; amp in Cx words
-constexpr int kColumnWords5 = 90 + 32;                                                              // Cx words per thread
+#ifndef HEGET_THREAD5_LEAN
+#define HEGET_THREAD5_LEAN 1   // fp64: the column holds P_{i} and P_{all\i} (5 + 5 entries) and the vectors v({i}, i, h) and
+                               // rows U_i(h) are recomputed where used (6 FMAs each): 1 632 instead of 1 952 B per thread,
+                               // i.e. 4 instead of 3 CTAs per SM: measured 1.60 -> 1.21 ms.  fp32 is not limited by shared
+                               // memory (0.613 -> 0.627 ms) and keeps the 10 + 10 vectors and rows themselves
+#endif
+// layout of the thread's column: spinor-sized slots (two Cx words each), then the 32 accumulators
+template <typename T>
+struct Col5 {
+    static constexpr bool LEAN = (HEGET_THREAD5_LEAN != 0) && (sizeof(T) == 8);
+    static constexpr int V1 = 0, U = LEAN ? 5 : 10, P2 = LEAN ? 10 : 20, P3 = P2 + 10, E = P3 + 10, AMP = 2 * (E + 5);
+    static constexpr int WORDS = AMP + 32;   // Cx words per thread
+};
+
+// v({i}, i, h) and U_i(h): read from the column, or rebuilt from the P entry kept there
+template <int CTA, typename T>
+__device__ __forceinline__ Spinor<T> v1_5(const Cx<T>* col, int i, int h, const EEntry<T>& e)
+{
+    if constexpr (Col5<T>::LEAN) {
+        const Cx<T> a = col[(2 * (Col5<T>::V1 + i)) * CTA], b = col[(2 * (Col5<T>::V1 + i) + 1) * CTA];
+        return chain_vector(PEntry<T>{a.r, a.i, b.r, b.i}, e);
+    } else {
+        const Cx<T> a = col[(2 * (Col5<T>::V1 + 2 * i + h)) * CTA], b = col[(2 * (Col5<T>::V1 + 2 * i + h) + 1) * CTA];
+        return {a.r, a.i, b.r, b.i};
+    }
+}
+template <int CTA, typename T>
+__device__ __forceinline__ Spinor<T> u_5(const Cx<T>* col, int i, int h, const EEntry<T>& e)
+{
+    if constexpr (Col5<T>::LEAN) {
+        const Cx<T> a = col[(2 * (Col5<T>::U + i)) * CTA], b = col[(2 * (Col5<T>::U + i) + 1) * CTA];
+        return closing_entry(e, PEntry<T>{a.r, a.i, b.r, b.i});
+    } else {
+        const Cx<T> a = col[(2 * (Col5<T>::U + 2 * i + h)) * CTA], b = col[(2 * (Col5<T>::U + 2 * i + h) + 1) * CTA];
+        return {a.r, a.i, b.r, b.i};
+    }
+}
 
 // the 10 units of work: triple {i < j < k} in colex order and the pair {a < b} left over
 struct Triple5 { unsigned char i, j, k, a, b; };
@@ -434,7 +469,7 @@ __constant__ Triple5 c_triples5[10] = {{0, 1, 2, 3, 4}, {0, 1, 3, 2, 4}, {0, 2, 
 template <int CTA, int H, typename T>
 __device__ __forceinline__ EEntry<T> e5(const Cx<T>* col, int ph)
 {
-    const Cx<T> a = col[(2 * (kCol5E + ph)) * CTA], b = col[(2 * (kCol5E + ph) + 1) * CTA];
+    const Cx<T> a = col[(2 * (Col5<T>::E + ph)) * CTA], b = col[(2 * (Col5<T>::E + ph) + 1) * CTA];
     if constexpr (H == 1) return {a.r, a.i, b.r, b.i};
     return {-b.r, b.i, -a.r, a.i};
 }
@@ -502,11 +537,16 @@ amp2_thread5_kernel(const double* __restrict__ momenta, double* __restrict__ out
         for (int i = 0; i < N; ++i) {
             const PEntry<T> p1 = kin.template subset<T>(1u << i);
             const PEntry<T> p4 = kin.template subset<T>(ALL ^ (1u << i));
+            if constexpr (Col5<T>::LEAN) {
+                put5<CTA>(col, Col5<T>::V1 + i, p1.pp, p1.pm, p1.px, p1.py);
+                put5<CTA>(col, Col5<T>::U + i, p4.pp, p4.pm, p4.px, p4.py);
+            } else {
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const Spinor<T> v = chain_vector(p1, e[i][h]), u = closing_entry(e[i][h], p4);
-                put5<CTA>(col, kCol5V1 + 2 * i + h, v.r0, v.i0, v.r1, v.i1);
-                put5<CTA>(col, kCol5U + 2 * i + h, u.r0, u.i0, u.r1, u.i1);
+                for (int h = 0; h < 2; ++h) {
+                    const Spinor<T> v = chain_vector(p1, e[i][h]), u = closing_entry(e[i][h], p4);
+                    put5<CTA>(col, Col5<T>::V1 + 2 * i + h, v.r0, v.i0, v.r1, v.i1);
+                    put5<CTA>(col, Col5<T>::U + 2 * i + h, u.r0, u.i0, u.r1, u.i1);
+                }
             }
         }
 #pragma unroll
@@ -514,7 +554,7 @@ amp2_thread5_kernel(const double* __restrict__ momenta, double* __restrict__ out
 #pragma unroll
             for (int i = 0; i < j; ++i) {
                 const PEntry<T> p = kin.template subset<T>((1u << i) | (1u << j));
-                put5<CTA>(col, kCol5P2 + j * (j - 1) / 2 + i, p.pp, p.pm, p.px, p.py);
+                put5<CTA>(col, Col5<T>::P2 + j * (j - 1) / 2 + i, p.pp, p.pm, p.px, p.py);
             }
 #pragma unroll
         for (int kk = 2; kk < N; ++kk)
@@ -523,12 +563,12 @@ amp2_thread5_kernel(const double* __restrict__ momenta, double* __restrict__ out
 #pragma unroll
                 for (int i = 0; i < j; ++i) {
                     const PEntry<T> p = kin.template subset<T>((1u << i) | (1u << j) | (1u << kk));
-                    put5<CTA>(col, kCol5P3 + kk * (kk - 1) * (kk - 2) / 6 + j * (j - 1) / 2 + i, p.pp, p.pm, p.px, p.py);
+                    put5<CTA>(col, Col5<T>::P3 + kk * (kk - 1) * (kk - 2) / 6 + j * (j - 1) / 2 + i, p.pp, p.pm, p.px, p.py);
                 }
 #pragma unroll
-        for (int i = 0; i < N; ++i) put5<CTA>(col, kCol5E + i, e[i][1].ar, e[i][1].ai, e[i][1].br, e[i][1].bi);
+        for (int i = 0; i < N; ++i) put5<CTA>(col, Col5<T>::E + i, e[i][1].ar, e[i][1].ai, e[i][1].br, e[i][1].bi);
 #pragma unroll
-        for (int h = 0; h < 32; ++h) col[(kCol5Amp + h) * CTA] = {(T)0, (T)0};
+        for (int h = 0; h < 32; ++h) col[(Col5<T>::AMP + h) * CTA] = {(T)0, (T)0};
     }
     __syncwarp();   // keeps the compiler from forwarding the column through registers (it would spill)
 
@@ -539,20 +579,20 @@ amp2_thread5_kernel(const double* __restrict__ momenta, double* __restrict__ out
     for (int t = 0; t < 10; ++t) {
         const int t3[3] = {c_triples5[t].i, c_triples5[t].j, c_triples5[t].k};
         const int a = c_triples5[t].a, b = c_triples5[t].b;
-        const PEntry<T> p3 = get5p<CTA>(col, kCol5P3 + t);
+        const PEntry<T> p3 = get5p<CTA>(col, Col5<T>::P3 + t);
         Spinor<T> psi[8];   // index 4 h_i + 2 h_j + h_k
 #pragma unroll
         for (int rr = 0; rr < 3; ++rr) {
             // last photon r of the prefix; p < q the other two: orderings (p, q, r) and (q, p, r)
             const int r = t3[2 - rr], p = t3[rr == 2 ? 1 : 0], q = t3[rr == 0 ? 1 : 2];
             const int sr = rr, sp = (rr == 2) ? 1 : 2, sq = (rr == 0) ? 1 : 0;   // bit of h_r, h_p, h_q in psi's index
-            const PEntry<T> p2 = get5p<CTA>(col, kCol5P2 + q * (q - 1) / 2 + p);
+            const PEntry<T> p2 = get5p<CTA>(col, Col5<T>::P2 + q * (q - 1) / 2 + p);
             const EEntry<T> ep[2] = {e5<CTA, 0>(col, p), e5<CTA, 1>(col, p)}, eq[2] = {e5<CTA, 0>(col, q), e5<CTA, 1>(col, q)},
                             er[2] = {e5<CTA, 0>(col, r), e5<CTA, 1>(col, r)};
             Cx<T> A[2][2], B[2][2], C[2][2], D[2][2];   // rho(p->q)[hp][hq], rho(q->r)[hq][hr], rho(q->p)[hq][hp], rho(p->r)[hp][hr]
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
-                const Spinor<T> v1p = get5<CTA>(col, kCol5V1 + 2 * p + h), v1q = get5<CTA>(col, kCol5V1 + 2 * q + h);
+                const Spinor<T> v1p = v1_5<CTA>(col, p, h, ep[h]), v1q = v1_5<CTA>(col, q, h, eq[h]);
                 const Spinor<T> v2q = chain_vector(p2, eq[h]), v2p = chain_vector(p2, ep[h]);   // last = q / p, helicity h
 #pragma unroll
                 for (int g2 = 0; g2 < 2; ++g2) {
@@ -586,13 +626,13 @@ amp2_thread5_kernel(const double* __restrict__ momenta, double* __restrict__ out
         }
         const EEntry<T> ea[2] = {e5<CTA, 0>(col, a), e5<CTA, 1>(col, a)}, eb[2] = {e5<CTA, 0>(col, b), e5<CTA, 1>(col, b)};
         // accumulator of assignment h sits at word h: bits of the triple's and the pair's photons, as byte offsets
-        Cx<T>* amp = col + kCol5Amp * CTA;
+        Cx<T>* amp = col + Col5<T>::AMP * CTA;
 #pragma unroll
         for (int ha = 0; ha < 2; ++ha) {
-            const Spinor<T> ua = get5<CTA>(col, kCol5U + 2 * a + ha);
+            const Spinor<T> ua = u_5<CTA>(col, a, ha, ea[ha]);
 #pragma unroll
             for (int hb = 0; hb < 2; ++hb) {
-                const Spinor<T> w = pair_row(ua, get5<CTA>(col, kCol5U + 2 * b + hb), ea[ha], eb[hb]);
+                const Spinor<T> w = pair_row(ua, u_5<CTA>(col, b, hb, eb[hb]), ea[ha], eb[hb]);
                 const int hab = (ha << a) | (hb << b);
                 // eight accumulators at a time: all loads, then all stores (the compiler must keep a load behind an
                 // earlier store it cannot tell apart, which would make the 32 updates of a triple one serial chain)
@@ -617,7 +657,7 @@ amp2_thread5_kernel(const double* __restrict__ momenta, double* __restrict__ out
     double m2 = 0.0;
 #pragma unroll
     for (int h = 0; h < 32; ++h) {
-        const Cx<T> acc = col[(kCol5Amp + h) * CTA];
+        const Cx<T> acc = col[(Col5<T>::AMP + h) * CTA];
         m2 += (double)acc.r * (double)acc.r + (double)acc.i * (double)acc.i;
     }
     if (live) out[ev] = norm * m2;
@@ -626,7 +666,7 @@ amp2_thread5_kernel(const double* __restrict__ momenta, double* __restrict__ out
 template <typename T>
 cudaError_t launch_thread5(const double* momenta, double* out, int64_t n_events, double g, cudaStream_t stream)
 {
-    constexpr size_t dyn = sizeof(Cx<T>) * kColumnWords5 * HEGET_THREAD5_CTA;
+    constexpr size_t dyn = sizeof(Cx<T>) * Col5<T>::WORDS * HEGET_THREAD5_CTA;
     const cudaError_t attr = cudaFuncSetAttribute(amp2_thread5_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
     if (attr != cudaSuccess) return attr;
     const int64_t blocks = (n_events + HEGET_THREAD5_CTA - 1) / HEGET_THREAD5_CTA;
