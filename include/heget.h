@@ -44,7 +44,8 @@ enum {
     HEGET_OK = 0,
     HEGET_EINVAL = -1, /* n outside [2,8], N < 0 or > HEGET_MAX_EVENTS, null pointer, bad precision/mode */
     HEGET_ECUDA = -2,  /* a CUDA runtime call or launch failed */
-    HEGET_ENOMEM = -3  /* host or device allocation failed */
+    HEGET_ENOMEM = -3, /* host or device allocation failed */
+    HEGET_ETOOBIG = -4 /* N exceeds the fixed scratch of a no-allocation entry point */
 };
 
 /* Largest N (events, or items of the heget_helas_* calls) one call accepts: the kernels that give
@@ -205,6 +206,23 @@ int heget_helas_vertex(heget_ctx* ctx, int fn, int precision, const double* fi, 
  *   amp2, weight [dev] const double[N]; out3 [dev] double[3], written. */
 int heget_xsec_reduce(heget_ctx* ctx, const double* amp2, const double* weight, int n, int64_t N,
                       double* out3, void* stream);
+
+/* heget_xsec_reduce for callers that cannot allocate and must not touch allocator-owned scratch: code under
+ * CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  Same arguments and result
+ * ({sum x, sum x^2, count}; a different, equally fixed reduction tree, so sums agree with heget_xsec_reduce to
+ * rounding, ~1e-15, and are bit-reproducible from call to call).  The block partials live in a file-scope
+ * `static __device__` array inside the library: 96 KB that every GPU which loads libheget.so holds until exit.
+ * It bounds the batch: N > HEGET_NOALLOC_MAX_EVENTS (2^24) returns HEGET_ETOOBIG (heget_last_cuda_error has
+ * the text).  The call launches two kernels on `stream` and calls no cudaMalloc / cudaFree / allocating
+ * routine; the first call on a device resolves the array's device address (cudaGetSymbolAddress, once per
+ * device) -- make one call before starting a graph capture.  All calls, from every context, share that one
+ * array and it keeps the last call's contents (nothing in it needs clearing: a call overwrites what it
+ * reads): calls that OVERLAP ON THE GPU -- different streams, concurrent graph launches -- race on it;
+ * order them on one stream or with events.
+ *   amp2, weight [dev] const double[N]; out3 [dev] double[3], written. */
+#define HEGET_NOALLOC_MAX_EVENTS 16777216LL
+int heget_xsec_reduce_noalloc(heget_ctx* ctx, const double* amp2, const double* weight, int n, int64_t N,
+                              double* out3, void* stream);
 
 /* End-to-end form of the same path with host buffers: copies momenta and weight to the
  * device, runs heget_amp2 and heget_xsec_reduce, copies out_amp2 (if non-NULL) and out3

@@ -19,7 +19,7 @@ VTX_IOVXXX, VTX_FVIXX0, VTX_FVOXX0, VTX_JIOXX0 = range(4)
 GEN_FIXED, GEN_LOGUNIFORM, GEN_TOYPDF = 0, 1, 2
 
 EXPORTS = ["heget_init", "heget_destroy", "heget_strerror", "heget_last_cuda_error", "heget_rambo",
-           "heget_gen_events", "heget_amp2", "heget_amp2_algo", "heget_amp2_sampled", "heget_list2", "heget_list2_sum", "heget_histogram", "heget_helas_wavefunction", "heget_helas_vertex", "heget_xsec_reduce", "heget_xsec_host", "heget_fma_peak", "heget_fma_peak_pattern",
+           "heget_gen_events", "heget_amp2", "heget_amp2_algo", "heget_amp2_sampled", "heget_list2", "heget_list2_sum", "heget_histogram", "heget_helas_wavefunction", "heget_helas_vertex", "heget_xsec_reduce", "heget_xsec_reduce_noalloc", "heget_xsec_host", "heget_fma_peak", "heget_fma_peak_pattern",
            "heget_launch_count"]
 
 
@@ -76,6 +76,8 @@ def load_library():
     lib.heget_helas_vertex.restype = ci
     lib.heget_xsec_reduce.argtypes = [vp, dp, dp, ci, i64, dp, vp]
     lib.heget_xsec_reduce.restype = ci
+    lib.heget_xsec_reduce_noalloc.argtypes = [vp, dp, dp, ci, i64, dp, vp]
+    lib.heget_xsec_reduce_noalloc.restype = ci
     lib.heget_xsec_host.argtypes = [vp, dp, dp, ci, ci, i64, dp, dp]
     lib.heget_xsec_host.restype = ci
     lib.heget_fma_peak.argtypes = [vp, ci, ctypes.POINTER(cd)]
@@ -242,6 +244,19 @@ class Heget:
         self._check(self._lib.heget_xsec_reduce(self._ctx, amp2.data_ptr(), weight.data_ptr(), n,
                                                 amp2.shape[0], out3.data_ptr(), _stream_ptr(self.device)),
                     "heget_xsec_reduce")
+        return out3
+
+    def xsec_reduce_noalloc(self, amp2, weight, n, out3):
+        """heget_xsec_reduce with its scratch in a static device array of the library: allocates nothing (the
+        caller passes out3), N <= 2^24 events, calls must not overlap on the GPU."""
+        _check_dev(amp2, None, self.device)
+        _check_dev(weight, amp2.shape, self.device)
+        _check_dev(out3, (3,), self.device)
+        rc = self._lib.heget_xsec_reduce_noalloc(self._ctx, amp2.data_ptr(), weight.data_ptr(), n, amp2.shape[0],
+                                                 out3.data_ptr(), _stream_ptr(self.device))
+        if rc == -4:
+            raise HegetError(self._lib.heget_strerror(rc).decode() + ": " + self._lib.heget_last_cuda_error(self._ctx).decode())
+        self._check(rc, "heget_xsec_reduce_noalloc")
         return out3
 
     def xsec_host(self, momenta, weight, precision=FP64, out_amp2=None, out3=None):

@@ -130,6 +130,7 @@ const char* heget_strerror(int code)
         case HEGET_EINVAL: return "invalid argument (n outside [2,8], N < 0 || N > HEGET_MAX_EVENTS, null pointer, bad precision or mode)";
         case HEGET_ECUDA: return "CUDA runtime error (see heget_last_cuda_error)";
         case HEGET_ENOMEM: return "allocation failed";
+        case HEGET_ETOOBIG: return "batch larger than the fixed scratch of a no-allocation entry point (N > HEGET_NOALLOC_MAX_EVENTS)";
         default: return "unknown heget error code";
     }
 }
@@ -287,6 +288,23 @@ int heget_xsec_reduce(heget_ctx* ctx, const double* amp2, const double* weight, 
     int launches = 0;
     double* partials = ctx->d_partials + (size_t)(ctx->reduce_slot++ % HEGET_REDUCE_SLOTS) * 3 * kReduceBlocks;
     cudaError_t err = heget_launch_reduce(partials, amp2, weight, n, N, out3, (cudaStream_t)stream, &launches);
+    ctx->launches += launches;
+    return err == cudaSuccess ? HEGET_OK : fail_cuda(ctx, err);
+}
+
+int heget_xsec_reduce_noalloc(heget_ctx* ctx, const double* amp2, const double* weight, int n, int64_t N, double* out3,
+                              void* stream)
+{
+    if (!ctx || n < 2 || n > 8 || N < 0 || !out3 || (N > 0 && (!amp2 || !weight))) return HEGET_EINVAL;
+    if (N > HEGET_NOALLOC_MAX_EVENTS) {
+        snprintf(ctx->cuda_msg, sizeof(ctx->cuda_msg), "heget_xsec_reduce_noalloc: N = %lld exceeds HEGET_NOALLOC_MAX_EVENTS = %lld",
+                 (long long)N, (long long)HEGET_NOALLOC_MAX_EVENTS);
+        return HEGET_ETOOBIG;
+    }
+    DeviceGuard guard(ctx->device);
+    if (!guard.ok) return fail_cuda(ctx, cudaGetLastError());
+    int launches = 0;
+    cudaError_t err = heget_launch_reduce_noalloc(ctx->device, amp2, weight, n, N, out3, (cudaStream_t)stream, &launches);
     ctx->launches += launches;
     return err == cudaSuccess ? HEGET_OK : fail_cuda(ctx, err);
 }

@@ -62,4 +62,6 @@ cudaError_t heget_launch_gen(const heget_ctx* ctx, uint64_t seed, int n, const h
                              cudaStream_t stream, int* launches);
 cudaError_t heget_launch_reduce(double* partials /* [kReduceBlocks][3] */, const double* amp2, const double* weight,
                                 int n, int64_t N, double* out3, cudaStream_t stream, int* launches);
+cudaError_t heget_launch_reduce_noalloc(int device /* current */, const double* amp2, const double* weight, int n, int64_t N,
+                                        double* out3, cudaStream_t stream, int* launches);
 cudaError_t heget_run_fma_peak(const heget_ctx* ctx, int precision, int pattern, double* flops_per_s, int* launches);

@@ -72,7 +72,78 @@ reduce_final_kernel(const double* __restrict__ partials, int n_partials, double*
     if (threadIdx.x == 0) { out3[0] = s1; out3[1] = s2; out3[2] = cnt; }
 }
 
+// ---- no-allocation variant (heget_xsec_reduce_noalloc) ---------------------------------------------------------
+// For callers that cannot call cudaMalloc (CUDA graph capture, serving loops, harnesses that forbid it) and do not
+// want a context-owned buffer either: the block partials live in a file-scope device array.  One block per chunk
+// of kNoAllocChunk events (no grid stride), one partial triple per block, so the scratch bounds the batch:
+// HEGET_NOALLOC_MAX_EVENTS = kNoAllocMaxBlocks * kNoAllocChunk.  Every GPU that loads the library holds the
+// 96 KB until exit.  All calls share the array and it keeps the last call's contents: a call writes partials
+// [0, blocks) before its final kernel reads exactly those, so nothing has to start at zero -- but two calls
+// that overlap on the GPU (different streams, or graphs launched concurrently) race on it.
+constexpr int kNoAllocChunk = 256 * 16;                                          // events per block
+constexpr int kNoAllocMaxBlocks = (int)(HEGET_NOALLOC_MAX_EVENTS / kNoAllocChunk);  // 4096
+static_assert((int64_t)kNoAllocMaxBlocks * kNoAllocChunk == HEGET_NOALLOC_MAX_EVENTS, "the maximum is a whole number of chunks");
+static __device__ __align__(256) double g_noalloc_partials[kNoAllocMaxBlocks * 3];
+
+__global__ void __launch_bounds__(256)
+reduce_partial_noalloc_kernel(const double* __restrict__ amp2, const double* __restrict__ weight, int64_t n_events,
+                              double factor, double* __restrict__ partials)
+{
+    __shared__ double sm[8][3];
+    double s1 = 0.0, s2 = 0.0, cnt = 0.0;
+    const int64_t lo = (int64_t)blockIdx.x * kNoAllocChunk;
+#pragma unroll 4
+    for (int k = 0; k < kNoAllocChunk / 256; ++k) {
+        const int64_t e = lo + k * 256 + threadIdx.x;
+        if (e < n_events) {
+            const double w = weight[e];
+            const double x = (w != 0.0) ? w * amp2[e] * factor : 0.0;   // DESIGN.md R26, as reduce_partial_kernel
+            s1 += x;
+            s2 += x * x;
+            cnt += (w != 0.0) ? 1.0 : 0.0;
+        }
+    }
+    block_sum3(s1, s2, cnt, sm);
+    if (threadIdx.x == 0) {
+        partials[3 * blockIdx.x + 0] = s1;
+        partials[3 * blockIdx.x + 1] = s2;
+        partials[3 * blockIdx.x + 2] = cnt;
+    }
+}
+
+// In host code `g_noalloc_partials` is a host-side stand-in, not a device address: the address a kernel can use
+// comes from cudaGetSymbolAddress, resolved once per device with that device current.
+constexpr int kMaxDevices = 64;
+double* g_noalloc_addr[kMaxDevices] = {};
+
 }  // namespace
+
+cudaError_t heget_launch_reduce_noalloc(int device, const double* amp2, const double* weight, int n, int64_t N,
+                                        double* out3, cudaStream_t stream, int* launches)
+{
+    *launches = 0;
+    if (device < 0 || device >= kMaxDevices) return cudaErrorInvalidDevice;
+    double* partials = g_noalloc_addr[device];
+    if (!partials) {   // set-up, once per device (the caller made `device` current); benign if two threads race: same value
+        void* p = nullptr;
+        const cudaError_t err = cudaGetSymbolAddress(&p, g_noalloc_partials);
+        if (err != cudaSuccess) return err;
+        g_noalloc_addr[device] = partials = static_cast<double*>(p);
+    }
+    double nfact = 1.0;
+    for (int i = 2; i <= n; ++i) nfact *= (double)i;
+    const double factor = kSpinAverage * kColourFactor / nfact;
+    const int blocks = (int)((N + kNoAllocChunk - 1) / kNoAllocChunk);   // <= kNoAllocMaxBlocks, checked by the caller
+    if (blocks > 0) {
+        reduce_partial_noalloc_kernel<<<blocks, 256, 0, stream>>>(amp2, weight, N, factor, partials);
+        const cudaError_t err = cudaGetLastError();
+        if (err != cudaSuccess) return err;
+        ++*launches;
+    }
+    reduce_final_kernel<<<1, 256, 0, stream>>>(partials, blocks, out3);   // blocks = 0: writes {0, 0, 0}
+    ++*launches;
+    return cudaGetLastError();
+}
 
 cudaError_t heget_launch_reduce(double* partials, const double* amp2, const double* weight, int n,
                                 int64_t N, double* out3, cudaStream_t stream, int* launches)
