@@ -140,10 +140,11 @@ def kernel_sass_sha(kernel, n, precision):
 
 
 def sass_flops_per_event(n, precision):
-    """Flops per event of the thread-per-event kernels (n <= 4), counted in the SASS of the library
-    that is loaded: those kernels are straight-line code executed once per event, so the static count
-    of {D,F}FMA (x2), {D,F}MUL, {D,F}ADD IS the executed count, tables included.  None if cuobjdump is
-    not available or the kernel has a loop."""
+    """Flops per event of the thread-per-event kernels (n <= 5), counted in the SASS of the library
+    that is loaded: those kernels are straight-line code executed once per event (n = 5: plus one rolled
+    loop over the 10 photon triples, whose body is weighted by its trip count), so the static count of
+    {D,F}FMA (x2), {D,F}MUL, {D,F}ADD IS the executed count, tables included.  None if cuobjdump is not
+    available or the control flow is not of that form."""
     if n > THREAD_MAXN:
         return None
     key = (n, precision)
