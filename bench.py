@@ -30,12 +30,13 @@ if ROOT not in sys.path:
 METRIC = "events/s of summed |M|^2 for u ubar->n gamma"
 UNIT = "events/s"
 ALGOS = {"tree": 0, "subset": 1, "two-sided": 2}
-THREAD_MAXN = 5     # n <= 5: one thread per event (csrc/amp2_thread.cu); n >= 6: one lane per helicity assignment
+THREAD_MAXN = 6     # n <= 5: one thread per event, n = 6: two / four lanes per event (csrc/amp2_thread.cu); n >= 7: one lane
+                    # per helicity assignment (csrc/amp2.cu)
 
 
 def kernel_name(algo, n):
     if algo == "tree":
-        return "amp2_kernel" if n > THREAD_MAXN else ("amp2_thread5_kernel" if n == 5 else "amp2_thread_kernel")
+        return "amp2_kernel" if n > THREAD_MAXN else ("amp2_thread%d_kernel" % n if n >= 5 else "amp2_thread_kernel")
     return {"subset": "amp2_subset_kernel", "two-sided": "amp2_twosided_kernel"}[algo]
 
 
@@ -51,7 +52,7 @@ def model_flops_per_event(n):
 
 def executed_flops_per_event(n, precision="fp32"):
     """What the tree kernels execute per event, tables excluded.
-    n >= 6 (lane per helicity assignment, factorised nodes psi = z v, csrc/amp2_chain.cuh): 2^n lanes;
+    n >= 7 (lane per helicity assignment, factorised nodes psi = z v, csrc/amp2_chain.cuh): 2^n lanes;
     every ordered prefix of up to n-4 photons is rho (4 FMA) + the vector v of the node (5 FMA + 1 MUL)
     + the accumulation rho A (4 FMA) = 27 flop; a prefix of n-3 photons needs no vector (the rho of its
     three children come from the per-event rho table, their closing dots from the K table): rho +
@@ -64,9 +65,13 @@ def executed_flops_per_event(n, precision="fp32"):
     n = 3: 6 vectors (11), 24 dots (16 + 2); n = 2: the closing rows only (counted with the tables).
     The kernels' whole count, tables included, is read from the SASS (sass_flops_per_event) or from the
     ncu summaries under profiles/."""
-    if n >= 6:
+    if n >= 7:
         upper = sum(math.factorial(n) // math.factorial(n - l) for l in range(1, n - 3))
         return 2 ** n * (27 * upper + 40 * (math.factorial(n) // 6))
+    if n == 6:
+        # two lanes per event, 15 photon quadruples each: 12 (last, third) blocks of ~400 flop (10 vectors, 5 rho
+        # tables, 8 products of two orderings, 8 accumulations), Psi 600, pair rows and 32 closing dots 912
+        return 2 * 15 * (12 * 400 + 600 + 912)
     if n == 5:
         return 10 * (18 * 11 + 48 * 8 + 48 * 16 + 4 * 32 + 32 * 18) + 20 * 11
     if n == 4:
@@ -119,7 +124,7 @@ def kernel_sass(kernel, n, precision):
         except Exception:
             _SASS_DUMP["text"] = []
     t = "d" if precision == "fp64" else "f"
-    want = "%sI%sE" % (kernel, t) if kernel == "amp2_thread5_kernel" else "%sILi%dE%s" % (kernel, n, t)
+    want = "%sI%sE" % (kernel, t) if kernel in ("amp2_thread5_kernel", "amp2_thread6_kernel") else "%sILi%dE%s" % (kernel, n, t)
     body, on = [], False
     for line in _SASS_DUMP["text"]:
         if "Function :" in line:
@@ -167,12 +172,16 @@ def sass_flops_per_event(n, precision):
                 if t and int(t.group(1), 16) <= addr:
                     loops.append((int(t.group(1), 16), addr))     # forward branches only skip a slow-path call
             ops.append((addr, op.split(".")[0]))
-        # n <= 4: no loop at all; n = 5: exactly one, the rolled loop over the 10 photon triples
-        trips = {5: 10}.get(n, 0)
-        if ops and ok and len(loops) == (1 if trips else 0):
+        # n <= 4: no loop at all; n = 5, 6: the rolled loop over the 10 photon triples / 15 quadruples; the fp64
+        # 6-photon kernel also keeps its loop over the 62 subsets rolled, two per trip.  Loops in program order.
+        trips = {(5, "fp64"): [10], (5, "fp32"): [10], (6, "fp32"): [15], (6, "fp64"): [31, 15]}.get((n, precision), [])
+        lanes = {6: 4 if precision == "fp64" else 2}.get(n, 1)      # lanes per event (HEGET_THREAD6_FIX64 / FIX32)
+        loops.sort(key=lambda lp: lp[1])
+        nested = any(a[0] <= b[0] <= a[1] for a in loops for b in loops if a is not b)
+        if ops and ok and len(loops) == len(trips) and not nested:
             w = {"DFMA": 2, "FFMA": 2, "DMUL": 1, "FMUL": 1, "DADD": 1, "FADD": 1}
-            inside = lambda a: bool(loops) and loops[0][0] <= a <= loops[0][1]
-            val = float(sum(w.get(o, 0) * (trips if inside(a) else 1) for a, o in ops))
+            mult = lambda a: next((tr for (lo, hi), tr in zip(loops, trips) if lo <= a <= hi), 1)
+            val = float(lanes * sum(w.get(o, 0) * mult(a) for a, o in ops))
     except Exception:
         val = None
     _SASS_CACHE[key] = val

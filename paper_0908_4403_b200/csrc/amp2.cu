@@ -16,6 +16,9 @@
 // |M(-sigma,-lambda)| = |M(sigma,lambda)|, so the helicity sum is twice the sum over lambda.
 #include "amp2_chain.cuh"
 
+#ifndef HEGET_THREAD_MAXN
+#define HEGET_THREAD_MAXN 6   // n up to this runs in amp2_thread.cu (5: 6 photons stay on the lane kernel below)
+#endif
 #ifndef HEGET_MINB32
 #define HEGET_MINB32 1      // fp32, n >= 6: __launch_bounds__ min CTAs of 256 threads per SM; 1 = no register cap (the six
                             // unrolled levels take 250 registers; capped at 128 they spill 600 B: 8 gamma 132 against 102 ms)
@@ -145,7 +148,7 @@ cudaError_t heget_launch_amp2(const heget_ctx* ctx, const double* momenta, int n
 {
     *launches = 0;
     if (N == 0) return cudaSuccess;
-    if (n <= 5) return heget_launch_amp2_thread(ctx, momenta, n, precision, out_amp2, N, stream, launches);
+    if (n <= HEGET_THREAD_MAXN) return heget_launch_amp2_thread(ctx, momenta, n, precision, out_amp2, N, stream, launches);
     *launches = 1;
     if (precision == HEGET_FP32) return launch_n<float>(ctx, n, momenta, out_amp2, N, ctx->g, stream);
     return launch_n<double>(ctx, n, momenta, out_amp2, N, ctx->g, stream);

@@ -1,4 +1,4 @@
-// amp2_thread.cu -- heget_amp2 for n = 2 .. 5: one THREAD per event (product code).
+// amp2_thread.cu -- heget_amp2 for n = 2 .. 6: one THREAD per event (n = 6: two or four lanes) (product code).
 //
 // This is the paper's own mapping (one phase-space point per thread) applied to the
 // permutation tree of eq. (6) in the two-component, factorised form of amp2_tables.cuh
@@ -682,6 +682,281 @@ cudaError_t launch_thread(const double* momenta, double* out, int64_t n_events, 
     return cudaGetLastError();
 }
 
+// ---- n = 6: TWO (fp32) or FOUR (fp64) adjacent lanes per event ------------------------------------------------------------------------
+//
+// The unit of work is a quadruple T4 = {t0 < t1 < t2 < t3} of photons with the pair {a, b} left over:
+//     Psi_T4(h) = sum over s in T4 of Y4(s; h) v(T4, s, h_s),
+//     Y4(s; h)  = sum over r in T4\s of [ z(p,q,r) + z(q,p,r) ] rho_s(v(T4\s, r, h_r)),   {p,q} = T4 \ {s,r},
+//     z(p,q,r)  = rho_q(v({p},p,h_p)) rho_r(v({p,q},q,h_q))      (every ordered prefix one product, as for n = 5)
+// closed by the pair rows: ampsum(h) += W_ab(h_a,h_b) . Psi_T4.  An event's 2^FIX lanes take the helicities of the
+// last FIX members of the quadruple (FIX = 1: t3; FIX = 2: t2 and t3): a lane holds Psi for the 2^(4-FIX)
+// assignments of the others and updates the 64 / 2^FIX accumulators with its helicities of the fixed ones.
+// fp64 uses FIX = 2: half the registers per lane (Psi, Y4 and the rho tables shrink) and twice the warps per SM.  Tables (the P entry of every subset, E' of lambda = +1) and the 64 accumulators
+// live in ONE column per event that both lanes address; which lane owns which accumulators changes from one
+// quadruple to the next, hence the __syncwarp() at the end of the loop body (a CTA is one warp).
+#ifndef HEGET_THREAD6_CTA
+#define HEGET_THREAD6_CTA 32   // threads per CTA = one warp (__syncwarp is the only synchronisation)
+#endif
+#ifndef HEGET_THREAD6_FIX32
+#define HEGET_THREAD6_FIX32 1  // lanes per event = 2^FIX
+#endif
+#ifndef HEGET_THREAD6_FIX64
+#define HEGET_THREAD6_FIX64 2  // fp64: measured 2^20 events: FIX = 1: 14.6 ms (255 registers, 750 B of spills, 4 warps per SM: the
+                               // column is 3 200 B per event), FIX = 2: 14.4 ms (254 registers, no spills, 8 warps per SM,
+                               // 1.4x the instructions: what does not depend on the fixed helicities is computed by every
+                               // lane).  Splitting the quadruples between two lane groups at FIX = 1 (own accumulators
+                               // each) was slower (18.7 ms), a register-lean order of the inner block no faster (15.0 ms)
+#endif
+#ifndef HEGET_THREAD6_MINB32
+#define HEGET_THREAD6_MINB32 8
+#endif
+#ifndef HEGET_THREAD6_MINB64
+#define HEGET_THREAD6_MINB64 8
+#endif
+struct Col6 {   // spinor-sized slots (two Cx words each), then the 64 accumulators
+    static constexpr int E = 0, P1 = 6, P5 = 12, P2 = 18, P3 = 33, P4 = 53, AMP = 2 * 68;   // followed by the 64 accumulators
+};
+struct Quad6 { unsigned char t[4], a, b; };   // at pair rank b (b - 1) / 2 + a: the complement of {a < b}
+__constant__ Quad6 c_quads6[15] = {{{2, 3, 4, 5}, 0, 1}, {{1, 3, 4, 5}, 0, 2}, {{0, 3, 4, 5}, 1, 2}, {{1, 2, 4, 5}, 0, 3}, {{0, 2, 4, 5}, 1, 3},
+                                   {{0, 1, 4, 5}, 2, 3}, {{1, 2, 3, 5}, 0, 4}, {{0, 2, 3, 5}, 1, 4}, {{0, 1, 3, 5}, 2, 4}, {{0, 1, 2, 5}, 3, 4},
+                                   {{1, 2, 3, 4}, 0, 5}, {{0, 2, 3, 4}, 1, 5}, {{0, 1, 3, 4}, 2, 5}, {{0, 1, 2, 4}, 3, 5}, {{0, 1, 2, 3}, 4, 5}};
+
+// positions 0..3 inside a quadruple: the last FIX positions have ONE helicity per lane and no bit in the index of Psi
+__host__ __device__ constexpr bool fixed6(int pos, int FIX) { return pos >= 4 - FIX; }
+__host__ __device__ constexpr int hc6(int pos, int FIX) { return fixed6(pos, FIX) ? 1 : 2; }
+__host__ __device__ constexpr int wt6(int pos, int FIX) { return fixed6(pos, FIX) ? 0 : (1 << (3 - FIX - pos)); }
+__host__ __device__ constexpr int wt6nz(int pos, int FIX) { return fixed6(pos, FIX) ? 1 : (1 << (3 - FIX - pos)); }
+__host__ __device__ constexpr int other6(int s, int k) { return k + (k >= s ? 1 : 0); }   // k-th position of T4 \ s
+
+template <int EV, typename T>
+__device__ __forceinline__ void put6(Cx<T>* col, int w, T a, T b, T c, T d)
+{
+    col[(2 * w) * EV] = {a, b};
+    col[(2 * w + 1) * EV] = {c, d};
+}
+template <int EV, typename T>
+__device__ __forceinline__ PEntry<T> getp6(const Cx<T>* col, int w)
+{
+    const Cx<T> a = col[(2 * w) * EV], b = col[(2 * w + 1) * EV];
+    return {a.r, a.i, b.r, b.i};
+}
+// E' entry of photon ph and helicity h (run time or folded) from the lambda = +1 entry in the column
+template <int EV, typename T>
+__device__ __forceinline__ EEntry<T> e6(const Cx<T>* col, int ph, int h)
+{
+    const Cx<T> a = col[(2 * (Col6::E + ph)) * EV], b = col[(2 * (Col6::E + ph) + 1) * EV];
+    return h ? EEntry<T>{a.r, a.i, b.r, b.i} : EEntry<T>{-b.r, b.i, -a.r, a.i};
+}
+
+template <typename T>
+constexpr int kFix6 = (sizeof(T) == 8) ? HEGET_THREAD6_FIX64 : HEGET_THREAD6_FIX32;
+
+template <typename T>
+__global__ void __launch_bounds__(HEGET_THREAD6_CTA, (sizeof(T) == 8) ? HEGET_THREAD6_MINB64 : HEGET_THREAD6_MINB32)
+amp2_thread6_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_t n_events, double g)
+{
+    constexpr int N = 6, FIX = kFix6<T>, LANES = 1 << FIX, EV = HEGET_THREAD6_CTA / LANES, NC = 1 << (4 - FIX);
+    constexpr unsigned ALL = 63u;
+    extern __shared__ __align__(16) unsigned char s_dyn6[];
+    Cx<T>* col = reinterpret_cast<Cx<T>*>(s_dyn6) + (threadIdx.x / LANES);
+    const int lane = threadIdx.x % LANES;   // bit 0: this lane's helicity of t3; bit 1 (FIX = 2): of t2
+    auto fixed_h = [lane](int pos) { return (lane >> (3 - pos)) & 1; };   // helicity of a fixed position
+
+    int64_t ev = (int64_t)blockIdx.x * EV + (threadIdx.x / LANES);
+    const bool live = ev < n_events;
+    if (!live) ev = n_events - 1;
+
+    double norm;
+    {   // prologue: both lanes of an event compute the tables (7 % of the kernel), each stores half of them
+        double e1, e2, k[N][4];
+        const double2* src = reinterpret_cast<const double2*>(momenta) + ev * (2 * (N + 2));
+        e1 = __ldg(src).x;
+        e2 = __ldg(src + 2).x;
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+            const double2 a = __ldg(src + 4 + 2 * i), b = __ldg(src + 5 + 2 * i);
+            k[i][0] = a.x; k[i][1] = a.y; k[i][2] = b.x; k[i][3] = b.y;
+        }
+        const double shat = 4.0 * e1 * e2;
+        const double scale = (sizeof(T) == 4) ? sqrt(shat) : 1.0;
+        norm = 2.0 * g * g * shat;
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+            EEntry<T> ep, em;
+            norm *= 0.5 * make_photon_entries<T>(k[i], &ep, &em);
+            if (lane == (i % LANES)) put6<EV>(col, Col6::E + i, ep.ar, ep.ai, ep.br, ep.bi);
+        }
+        if constexpr (sizeof(T) == 4) {
+            const double inv = 1.0 / shat;
+#pragma unroll
+            for (int i = 0; i < N - 1; ++i) norm *= inv;
+        }
+        Kinematics<N, sizeof(T) == 8> kin;
+        kin.init(k, e1, g, scale);
+#pragma unroll
+        for (unsigned S = 1; S < ALL; ++S) {
+            const int m = __popc(S);
+            // slot of subset S: singles and their complements by photon, pairs and quadruples by the rank of
+            // the (complementary) pair, triples by colex rank
+            int x = -1, y = -1, z = -1, cnt = 0;
+            const unsigned Q = (m <= 3) ? S : (ALL ^ S);   // the set that is ranked (at most 3 members)
+#pragma unroll
+            for (int i = 0; i < N; ++i)
+                if ((Q >> i) & 1u) { if (cnt == 0) x = i; else if (cnt == 1) y = i; else z = i; ++cnt; }
+            const int slot = (m == 1) ? Col6::P1 + x : (m == 5) ? Col6::P5 + x
+                           : (m == 2) ? Col6::P2 + y * (y - 1) / 2 + x : (m == 4) ? Col6::P4 + y * (y - 1) / 2 + x
+                           : Col6::P3 + z * (z - 1) * (z - 2) / 6 + y * (y - 1) / 2 + x;
+            const PEntry<T> pe = kin.template subset<T>(S);
+            if (lane == (int)(S % LANES)) put6<EV>(col, slot, pe.pp, pe.pm, pe.px, pe.py);
+        }
+#pragma unroll
+        for (int h = 0; h < 64 / LANES; ++h) col[(Col6::AMP + LANES * h + lane) * EV] = {(T)0, (T)0};
+    }
+    __syncwarp();
+
+#pragma unroll 1
+    for (int t = 0; t < 15; ++t) {
+        const int ph[4] = {c_quads6[t].t[0], c_quads6[t].t[1], c_quads6[t].t[2], c_quads6[t].t[3]};
+        const int a = c_quads6[t].a, b = c_quads6[t].b;
+        const PEntry<T> p4 = getp6<EV>(col, Col6::P4 + t);
+        Spinor<T> psi[NC];   // index: the helicities of the free positions, t0 most significant
+#pragma unroll
+        for (int sp = 0; sp < 4; ++sp) {   // s = last photon of the prefix, at position sp of the quadruple
+            const int x = ph[other6(sp, 0)], y = ph[other6(sp, 1)], z = ph[other6(sp, 2)];   // T4 \ s, increasing
+            const PEntry<T> p3 = getp6<EV>(col, Col6::P3 + z * (z - 1) * (z - 2) / 6 + y * (y - 1) / 2 + x);
+            const EEntry<T> es[2] = {e6<EV>(col, ph[sp], fixed6(sp, FIX) ? fixed_h(sp) : 0), e6<EV>(col, ph[sp], 1)};
+            Cx<T> y4[NC];
+#pragma unroll
+            for (int c = 0; c < NC; ++c) y4[c] = {(T)0, (T)0};
+#pragma unroll
+            for (int rk = 0; rk < 3; ++rk) {   // r = third photon; p < q the first two, in both orders
+                const int rp = other6(sp, rk), pp = other6(sp, rk == 0 ? 1 : 0), qp = other6(sp, rk == 2 ? 1 : 2);
+                const int r = ph[rp], p = ph[pp], q = ph[qp];
+                const EEntry<T> er[2] = {e6<EV>(col, r, fixed6(rp, FIX) ? fixed_h(rp) : 0), e6<EV>(col, r, 1)};
+                const EEntry<T> ep[2] = {e6<EV>(col, p, fixed6(pp, FIX) ? fixed_h(pp) : 0), e6<EV>(col, p, 1)};
+                const EEntry<T> eq[2] = {e6<EV>(col, q, fixed6(qp, FIX) ? fixed_h(qp) : 0), e6<EV>(col, q, 1)};
+                const PEntry<T> p2 = getp6<EV>(col, Col6::P2 + q * (q - 1) / 2 + p);
+                const PEntry<T> p1p = getp6<EV>(col, Col6::P1 + p), p1q = getp6<EV>(col, Col6::P1 + q);
+                Cx<T> A[2][2], B[2][2], C[2][2], D[2][2], R3[2][2];
+                // A = rho(p->q)[hp][hq], C = rho(q->p)[hq][hp], B = rho(q->r)[hq][hr], D = rho(p->r)[hp][hr], R3 = rho(r->s)[hr][hs]
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    if (h < hc6(pp, FIX)) {
+                        const Spinor<T> v1p = chain_vector(p1p, ep[h]), v2p = chain_vector(p2, ep[h]);
+#pragma unroll
+                        for (int g2 = 0; g2 < 2; ++g2) {
+                            if (g2 < hc6(qp, FIX)) chain_rho(v1p, eq[g2], A[h][g2].r, A[h][g2].i);
+                            if (g2 < hc6(rp, FIX)) chain_rho(v2p, er[g2], D[h][g2].r, D[h][g2].i);
+                        }
+                    }
+                    if (h < hc6(qp, FIX)) {
+                        const Spinor<T> v1q = chain_vector(p1q, eq[h]), v2q = chain_vector(p2, eq[h]);
+#pragma unroll
+                        for (int g2 = 0; g2 < 2; ++g2) {
+                            if (g2 < hc6(pp, FIX)) chain_rho(v1q, ep[g2], C[h][g2].r, C[h][g2].i);
+                            if (g2 < hc6(rp, FIX)) chain_rho(v2q, er[g2], B[h][g2].r, B[h][g2].i);
+                        }
+                    }
+                    if (h < hc6(rp, FIX)) {
+                        const Spinor<T> v3 = chain_vector(p3, er[h]);
+#pragma unroll
+                        for (int g2 = 0; g2 < 2; ++g2)
+                            if (g2 < hc6(sp, FIX)) chain_rho(v3, es[g2], R3[h][g2].r, R3[h][g2].i);
+                    }
+                }
+#pragma unroll
+                for (int hp = 0; hp < hc6(pp, FIX); ++hp)
+#pragma unroll
+                    for (int hq = 0; hq < hc6(qp, FIX); ++hq)
+#pragma unroll
+                        for (int hr = 0; hr < hc6(rp, FIX); ++hr) {
+                            Cx<T> zz = cx_mul(A[hp][hq], B[hq][hr]);                                         // (p, q, r)
+                            chain_acc(C[hq][hp].r, C[hq][hp].i, D[hp][hr].r, D[hp][hr].i, zz.r, zz.i);      // (q, p, r)
+#pragma unroll
+                            for (int hs = 0; hs < hc6(sp, FIX); ++hs) {
+                                Cx<T>& yy = y4[hp * wt6(pp, FIX) + hq * wt6(qp, FIX) + hr * wt6(rp, FIX) + hs * wt6(sp, FIX)];
+                                chain_acc(zz.r, zz.i, R3[hr][hs].r, R3[hr][hs].i, yy.r, yy.i);              // (.., r, s)
+                            }
+                        }
+            }
+#pragma unroll
+            for (int hs = 0; hs < hc6(sp, FIX); ++hs) {
+                const Spinor<T> v4 = chain_vector(p4, es[hs]);
+#pragma unroll
+                for (int c = 0; c < NC; ++c) {
+                    if (!fixed6(sp, FIX) && ((c / wt6nz(sp, FIX)) & 1) != hs) continue;   // c carries h_s unless s is fixed
+                    if (sp == 0) {
+                        psi[c].r0 = fma(y4[c].r, v4.r0, -(y4[c].i * v4.i0));
+                        psi[c].i0 = fma(y4[c].r, v4.i0, y4[c].i * v4.r0);
+                        psi[c].r1 = fma(y4[c].r, v4.r1, -(y4[c].i * v4.i1));
+                        psi[c].i1 = fma(y4[c].r, v4.i1, y4[c].i * v4.r1);
+                    } else {
+                        chain_acc(y4[c].r, y4[c].i, v4.r0, v4.i0, psi[c].r0, psi[c].i0);
+                        chain_acc(y4[c].r, y4[c].i, v4.r1, v4.i1, psi[c].r1, psi[c].i1);
+                    }
+                }
+            }
+        }
+        // close with the pair rows W_ab(h_a, h_b); this lane owns the accumulators with its helicities of the fixed positions
+        const EEntry<T> ea[2] = {e6<EV>(col, a, 0), e6<EV>(col, a, 1)}, eb[2] = {e6<EV>(col, b, 0), e6<EV>(col, b, 1)};
+        const PEntry<T> p5a = getp6<EV>(col, Col6::P5 + a), p5b = getp6<EV>(col, Col6::P5 + b);
+        Cx<T>* amp = col + Col6::AMP * EV;
+        int hfix = 0;
+#pragma unroll
+        for (int pos = 4 - FIX; pos < 4; ++pos) hfix |= fixed_h(pos) << ph[pos];
+        int hfree[NC];   // accumulator bits of the free positions for every index of Psi
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            hfree[c] = 0;
+#pragma unroll
+            for (int pos = 0; pos < 4 - FIX; ++pos) hfree[c] |= ((c / wt6nz(pos, FIX)) & 1) << ph[pos];
+        }
+#pragma unroll
+        for (int ha = 0; ha < 2; ++ha) {
+            const Spinor<T> ua = closing_entry(ea[ha], p5a);
+#pragma unroll
+            for (int hb = 0; hb < 2; ++hb) {
+                const Spinor<T> w = pair_row(ua, closing_entry(eb[hb], p5b), ea[ha], eb[hb]);
+                const int hab = (ha << a) | (hb << b) | hfix;
+                Cx<T> acc[NC];   // all loads, then all stores (see amp2_thread5_kernel)
+#pragma unroll
+                for (int c = 0; c < NC; ++c) acc[c] = amp[(hfree[c] | hab) * EV];
+#pragma unroll
+                for (int c = 0; c < NC; ++c) {
+                    const Cx<T> dot = row_dot(w, psi[c]);
+                    acc[c].r += dot.r;
+                    acc[c].i += dot.i;
+                }
+#pragma unroll
+                for (int c = 0; c < NC; ++c) amp[(hfree[c] | hab) * EV] = acc[c];
+            }
+        }
+        __syncwarp();   // the next quadruple splits the accumulators between the lanes differently
+    }
+
+    double m2 = 0.0;
+#pragma unroll
+    for (int h = lane; h < 64; h += LANES) {
+        const Cx<T> acc = col[(Col6::AMP + h) * EV];
+        m2 += (double)acc.r * (double)acc.r + (double)acc.i * (double)acc.i;
+    }
+#pragma unroll
+    for (int off = 1; off < LANES; off <<= 1) m2 += __shfl_xor_sync(0xffffffffu, m2, off);
+    if (live && lane == 0) out[ev] = norm * m2;
+}
+
+template <typename T>
+cudaError_t launch_thread6(const double* momenta, double* out, int64_t n_events, double g, cudaStream_t stream)
+{
+    constexpr int EV = HEGET_THREAD6_CTA >> kFix6<T>;
+    constexpr size_t dyn = sizeof(Cx<T>) * (Col6::AMP + 64) * EV;
+    const cudaError_t attr = cudaFuncSetAttribute(amp2_thread6_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
+    if (attr != cudaSuccess) return attr;
+    const int64_t blocks = (n_events + EV - 1) / EV;
+    amp2_thread6_kernel<T><<<(unsigned)blocks, HEGET_THREAD6_CTA, dyn, stream>>>(momenta, out, n_events, g);
+    return cudaGetLastError();
+}
+
 }  // namespace
 
 cudaError_t heget_launch_amp2_thread(const heget_ctx* ctx, const double* momenta, int n, int precision,
@@ -700,6 +975,8 @@ cudaError_t heget_launch_amp2_thread(const heget_ctx* ctx, const double* momenta
                            : launch_thread<4, double>(momenta, out_amp2, N, ctx->g, stream);
         case 5: return f32 ? launch_thread5<float>(momenta, out_amp2, N, ctx->g, stream)
                            : launch_thread5<double>(momenta, out_amp2, N, ctx->g, stream);
+        case 6: return f32 ? launch_thread6<float>(momenta, out_amp2, N, ctx->g, stream)
+                           : launch_thread6<double>(momenta, out_amp2, N, ctx->g, stream);
         default: return cudaErrorInvalidValue;
     }
 }

@@ -39,7 +39,7 @@ def test_flop_models_match_the_node_counts_of_the_survey():
     for n, nodes in internal.items():
         assert bench.model_flops_per_event(n) == 2 * 2 ** n * (44 * nodes + 24 * math.factorial(n))
         upper = nodes - math.factorial(n)            # prefixes of up to n-2 photons
-        if n >= 6:   # lane per helicity assignment: 27 flop per factorised node down to n-4 photons, 40 per node of n-3
+        if n >= 7:   # lane per helicity assignment: 27 flop per factorised node down to n-4 photons, 40 per node of n-3
             deep2, deep3 = math.factorial(n) // 2, math.factorial(n) // 6     # prefixes of exactly n-2 / n-3 photons
             assert bench.executed_flops_per_event(n, "fp32") == 2 ** n * (27 * (upper - deep2 - deep3) + 40 * deep3)
         else:        # thread per event: prefixes shared between helicity assignments, far below one tree per assignment
