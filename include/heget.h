@@ -112,8 +112,8 @@ int heget_gen_events(heget_ctx* ctx, uint64_t seed, int n, const heget_gen_cfg* 
  * (the two orderings below a prefix of n-2 photons are closed together
  * through a per-event table built from the ubar side; each fvixx0 of the walk is evaluated in
  * factorised form, a complex number times a per-(subset, photon) vector, which the rank-one
- * polarisation blocks of massless photons allow; n <= 5: one thread per event, n >= 6: one
- * lane per photon-helicity assignment), squared and
+ * polarisation blocks of massless photons allow; n <= 5: one thread per event, n = 6: two or
+ * four lanes per event, n >= 7: one lane per photon-helicity assignment), squared and
  * summed over all 4*2^n helicities:
  *   out_amp2[e] = sum_{sigma1,sigma2,lambda_1..lambda_n} |M|^2   (the sum in eq. 2,
  *   PAPER.md:37, WITHOUT 1/(2 s_hat), spin/colour average and 1/n!).

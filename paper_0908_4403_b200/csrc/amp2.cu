@@ -1,6 +1,7 @@
 // amp2.cu -- heget_amp2: summed squared helicity amplitude of u ubar -> n gamma (product code).
 //
-// n <= 5 runs one thread per event (amp2_thread.cu).  This file is the kernel for n >= 6:
+// n <= 6 runs in amp2_thread.cu (one thread, at n = 6 two or four lanes, per event).  This file is the kernel for
+// n >= 7 (it is instantiated for n = 6 too: HEGET_THREAD_MAXN = 5 puts 6 photons back on it):
 // one lane per photon-helicity configuration (2^N lanes per event), one event per CTA of 2^N
 // threads.  All lanes of a CTA walk the SAME
 // permutation tree in lockstep (no divergence); they differ only in which helicity entry of the
