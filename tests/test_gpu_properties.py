@@ -88,7 +88,7 @@ def test_algorithms_agree_on_every_event_of_the_headline_launch(hg):
 
 
 @pytest.mark.parametrize("n,N", [(2, (1 << 18) + 37), (3, (1 << 19) + 37), (4, (1 << 18) + 61), (5, (1 << 18) + 5),
-                                 (7, (1 << 13) + 1)])
+                                 (6, (1 << 16) + 13), (7, (1 << 13) + 1)])
 def test_three_organisations_of_the_sum_agree_on_large_ragged_batches(hg, n, N):
     """The one-sided tree (thread per event for n <= 4, lane per helicity assignment above), two-sided chaining
     and the subset recursion are three different evaluation orders of the same n! diagrams: on every event of
