@@ -85,3 +85,23 @@ def test_headline_line_carries_the_contract_and_a_fresh_ncu_summary():
     sys.path.insert(0, ROOT)
     import bench
     assert abs(bench.sass_flops_per_event(4, "fp64") / r["flops_per_event"] - 1.0) < 0.01
+
+
+def test_committed_ncu_summaries_describe_the_kernels_built_from_this_source():
+    """Every profiles/r02_amp2_<config>_<precision>.txt carries the hash of the SASS of the kernel it was captured
+    from; the library built from the source at hand must contain exactly that kernel (the build is deterministic),
+    otherwise the summary is stale and bench.py would refuse it."""
+    import re
+    sys.path.insert(0, ROOT)
+    import bench
+    from paper_0908_4403_b200 import build, workloads
+    build.build()
+    for name in workloads.ORDER:
+        n = workloads.CONFIGS[name]["n"]
+        for precision in ("fp64", "fp32"):
+            text = open(os.path.join(ROOT, "profiles", "r02_amp2_%s_%s.txt" % (name, precision))).read()
+            m = re.search(r"^sass_sha256: ([0-9a-f]+)", text, re.M)
+            assert m, (name, precision)
+            kernel = bench.kernel_name("tree", n)
+            assert re.search(r"^kernel: .*?%s<" % kernel, text, re.M), (name, precision, kernel)
+            assert bench.kernel_sass_sha(kernel, n, precision) == m.group(1), (name, precision)
