@@ -756,6 +756,7 @@ __global__ void __launch_bounds__(HEGET_THREAD6_CTA, (sizeof(T) == 8) ? HEGET_TH
 amp2_thread6_kernel(const double* __restrict__ momenta, double* __restrict__ out, int64_t n_events, double g)
 {
     constexpr int N = 6, FIX = kFix6<T>, LANES = 1 << FIX, EV = HEGET_THREAD6_CTA / LANES, NC = 1 << (4 - FIX);
+    static_assert(HEGET_THREAD6_CTA == 32 && (FIX == 1 || FIX == 2), "a CTA is one warp: __syncwarp() is the only synchronisation");
     constexpr unsigned ALL = 63u;
     extern __shared__ __align__(16) unsigned char s_dyn6[];
     Cx<T>* col = reinterpret_cast<Cx<T>*>(s_dyn6) + (threadIdx.x / LANES);
