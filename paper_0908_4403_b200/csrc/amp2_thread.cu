@@ -691,9 +691,10 @@ cudaError_t launch_thread(const double* momenta, double* out, int64_t n_events, 
 // closed by the pair rows: ampsum(h) += W_ab(h_a,h_b) . Psi_T4.  An event's 2^FIX lanes take the helicities of the
 // last FIX members of the quadruple (FIX = 1: t3; FIX = 2: t2 and t3): a lane holds Psi for the 2^(4-FIX)
 // assignments of the others and updates the 64 / 2^FIX accumulators with its helicities of the fixed ones.
-// fp64 uses FIX = 2: half the registers per lane (Psi, Y4 and the rho tables shrink) and twice the warps per SM.  Tables (the P entry of every subset, E' of lambda = +1) and the 64 accumulators
-// live in ONE column per event that both lanes address; which lane owns which accumulators changes from one
-// quadruple to the next, hence the __syncwarp() at the end of the loop body (a CTA is one warp).
+// fp64 uses FIX = 2: half the registers per lane (Psi, Y4 and the rho tables shrink) and twice the warps per SM.
+// Tables (the P entry of every subset, E' of lambda = +1) and the 64 accumulators live in ONE column per event
+// that all its lanes address; which lane owns which accumulators changes from one quadruple to the next, hence
+// the __syncwarp() at the end of the loop body (a CTA is one warp).
 #ifndef HEGET_THREAD6_CTA
 #define HEGET_THREAD6_CTA 32   // threads per CTA = one warp (__syncwarp is the only synchronisation)
 #endif
