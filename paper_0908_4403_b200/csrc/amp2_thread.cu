@@ -54,12 +54,16 @@ __device__ __forceinline__ void dd_add_to(dd& a, const dd& b)
 }
 
 // a.b = a0 b0 - a1 b1 - a2 b2 - a3 b3 as an unevaluated sum: exact products (FMA), the high parts
-// summed by TwoSum, every rounding error collected in lo
+// summed error-free, every rounding error collected in lo.  For two massless vectors (photons) the running sum
+// dominates the next term -- a0 b0 - a1 b1 >= |a2 b2| + |a3 b3| and a0 b0 - a1 b1 - a2 b2 >= |a3 b3| by
+// Cauchy-Schwarz on (|a1|,|a2|,|a3|).(|b1|,|b2|,|b3|) <= a0 b0 -- so the three additions are Dekker's
+// FastTwoSum (3 operations) instead of Knuth's TwoSum (6); an ulp-level violation from the rounding of the
+// running sum only moves a second-order error
 __device__ __forceinline__ dd dd_minkowski(const double (&a)[4], const double (&b)[4])
 {
     const dd p0 = dd_two_prod(a[0], b[0]), p1 = dd_two_prod(a[1], b[1]), p2 = dd_two_prod(a[2], b[2]),
              p3 = dd_two_prod(a[3], b[3]);
-    const dd s1 = dd_two_sum(p0.hi, -p1.hi), s2 = dd_two_sum(s1.hi, -p2.hi), s3 = dd_two_sum(s2.hi, -p3.hi);
+    const dd s1 = dd_fast_two_sum(p0.hi, -p1.hi), s2 = dd_fast_two_sum(s1.hi, -p2.hi), s3 = dd_fast_two_sum(s2.hi, -p3.hi);
     const double lo = __dadd_rn(__dadd_rn(__dsub_rn(__dsub_rn(__dsub_rn(p0.lo, p1.lo), p2.lo), p3.lo), s1.lo),
                                 __dadd_rn(s2.lo, s3.lo));
     return {s3.hi, lo};
