@@ -285,7 +285,7 @@ def test_two_photon_cross_section_closed_form_on_gpu(hg):
     assert abs(cnt / N - c) < 4 * math.sqrt(c * (1 - c) / N)
 
 
-FULL_SAMPLES = {"2gamma": 4096, "3gamma": 1024, "4gamma": 512, "5gamma": 64}
+FULL_SAMPLES = {"2gamma": 4096, "3gamma": 4096, "4gamma": 4096, "5gamma": 512}
 GOLDEN = __import__("os").path.join(__import__("os").path.dirname(__file__), "golden")
 
 
