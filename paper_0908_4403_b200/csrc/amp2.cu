@@ -63,8 +63,8 @@ constexpr bool kEByPtr = (sizeof(T) == 8) && (HEGET_CHAIN_E_BY_PTR64 != 0) && (k
 template <int N, typename T>
 struct ChainTables {
     static constexpr int NW = 4 * (N * (N - 1) / 2);          // pair closing rows W
-    static constexpr int NK = kChainEntries<N>;               // closing dots K
-    static constexpr int NR = kRhoEntries<N>;                 // rho of the last attachment
+    static constexpr int NK = kChainEntries<N, T>;            // closing dots K
+    static constexpr int NR = kRhoEntries<N, T>;              // rho of the last attachment
     static constexpr size_t BYTES = (size_t)TreeGeometry<N>::EPB * (NK + NR) * sizeof(Cx<T>);
 };
 

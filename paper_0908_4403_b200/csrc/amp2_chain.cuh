@@ -100,9 +100,32 @@ __device__ __forceinline__ void lds_cx3(unsigned addr, Cx<double>& a, Cx<double>
     asm volatile("ld.shared.v2.f64 {%0, %1}, [%2+256];" : "=d"(c.r), "=d"(c.i) : "r"(addr));
 }
 
-// K table entries per event: [triple T (colex rank)][slot of j in T][4 h_x + 2 h_y + h_z]
-template <int N>
-constexpr int kChainEntries = (N * (N - 1) * (N - 2) / 6) * 24;
+// fp32 "packed" layout (HEGET_CHAIN_PACKED32): the three entries a node of n-3 photons reads from the K table,
+// and the three it reads from the rho table, are ADJACENT (one 16-byte and one 8-byte load at constant offsets
+// from one lane-dependent address) instead of three loads at three lane-dependent addresses: a row holds, for
+// each of the 8 helicity assignments h_T = 4 h_x + 2 h_y + h_z of the triple, a chunk of 4 entries (3 used);
+// the chunks of h_T >= 4 are shifted by 2 entries so that the 8 chunks a warp reads at once fall into distinct
+// banks.  The rho table grows 4x (the rho of photon j is stored under every assignment of the other two), which
+// fp32 can afford (n = 8: 152 KB) and fp64 cannot.
+#ifndef HEGET_CHAIN_PACKED32
+#define HEGET_CHAIN_PACKED32 1
+#endif
+template <typename T>
+constexpr bool kPacked = (sizeof(T) == 4) && (HEGET_CHAIN_PACKED32 != 0);
+constexpr unsigned kPackRow = 8 * 4 + 2;                                   // entries per row
+__host__ __device__ constexpr unsigned pack_off(unsigned ht) { return 4u * ht + (ht >= 4u ? 2u : 0u); }
+
+// packed fp32: three adjacent entries
+__device__ __forceinline__ void lds_cx3_packed(unsigned addr, Cx<float>& a, Cx<float>& b, Cx<float>& c)
+{
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(a.r), "=f"(a.i), "=f"(b.r), "=f"(b.i) : "r"(addr));
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2+16];" : "=f"(c.r), "=f"(c.i) : "r"(addr));
+}
+__device__ __forceinline__ void lds_cx3_packed(unsigned, Cx<double>&, Cx<double>&, Cx<double>&) {}   // never used
+
+// K table entries per event: [triple T (colex rank)][slot of j in T][4 h_x + 2 h_y + h_z]; packed: [T][h_T chunk][slot]
+template <int N, typename T>
+constexpr int kChainEntries = (N * (N - 1) * (N - 2) / 6) * (kPacked<T> ? (int)kPackRow : 24);
 
 // unrank a photon triple x < y < z from its colex rank tr = C(z,3) + C(y,2) + x
 __device__ __forceinline__ void unrank_triple(unsigned tr, unsigned& x, unsigned& y, unsigned& z)
@@ -128,7 +151,7 @@ __device__ __forceinline__ void build_chain_table(const PEntry<T>* s_P, const EE
     const PEntry<T>* P = s_P + ev_local * G::L;
     const EEntry<T>* E = s_E + ev_local * 2 * N;
     const Spinor<T>* W = s_W + ev_local * 4 * (N * (N - 1) / 2);
-    Cx<T>* K = s_K + ev_local * kChainEntries<N>;
+    Cx<T>* K = s_K + ev_local * kChainEntries<N, T>;
     for (unsigned q = lane; q < ITEMS; q += G::L) {
         const unsigned hj = q & 1u, t = q >> 1, slot = t % 3u, tr = t / 3u;
         unsigned x, y, z;
@@ -145,15 +168,20 @@ __device__ __forceinline__ void build_chain_table(const PEntry<T>* s_P, const EE
             Cx<T> k;
             k.r = fma(w.r0, v.r0, fma(-w.i0, v.i0, fma(w.r1, v.r1, -(w.i1 * v.i1))));
             k.i = fma(w.r0, v.i0, fma(w.i0, v.r0, fma(w.r1, v.i1, w.i1 * v.r1)));
-            K[(tr * 3u + slot) * 8u + wj * hj + wa * (h >> 1) + wb * (h & 1u)] = k;
+            const unsigned ht = wj * hj + wa * (h >> 1) + wb * (h & 1u);
+            if constexpr (kPacked<T>)
+                K[tr * kPackRow + pack_off(ht) + slot] = k;
+            else
+                K[(tr * 3u + slot) * 8u + ht] = k;
         }
     }
     __syncthreads();
 }
 
-// rho table entries per event: [triple T (colex rank)][i: rank of i in all \ T][h_i][j: rank in T][h_j]
-template <int N>
-constexpr int kRhoEntries = (N * (N - 1) * (N - 2) / 6) * 12 * (N - 3);
+// rho table entries per event: [triple T (colex rank)][i: rank of i in all \ T][h_i][j: rank in T][h_j];
+// packed: [T][i][h_i] rows of [h_T chunk][j]
+template <int N, typename T>
+constexpr int kRhoEntries = (N * (N - 1) * (N - 2) / 6) * (N - 3) * (kPacked<T> ? 2 * (int)kPackRow : 12);
 
 // Reads s_P and s_E (barrier before), ends with a barrier.  One work item per (T, i, h_i): the vector
 // v(all \ T, i, h_i) once, then its six rho (j in T, h_j).
@@ -165,7 +193,7 @@ __device__ __forceinline__ void build_rho_table(const PEntry<T>* s_P, const EEnt
     const unsigned lane = threadIdx.x % G::L;
     const PEntry<T>* P = s_P + ev_local * G::L;
     const EEntry<T>* E = s_E + ev_local * 2 * N;
-    Cx<T>* R = s_R + ev_local * kRhoEntries<N>;
+    Cx<T>* R = s_R + ev_local * kRhoEntries<N, T>;
     for (unsigned q = lane; q < ITEMS; q += G::L) {
         const unsigned hi = q & 1u, t = q >> 1, islot = t % (N - 3), tr = t / (N - 3);
         unsigned x, y, z;
@@ -182,7 +210,14 @@ __device__ __forceinline__ void build_rho_table(const PEntry<T>* s_P, const EEnt
             for (unsigned hj = 0; hj < 2; ++hj) {
                 Cx<T> r;
                 chain_rho(v, E[2 * js[jslot] + hj], r.r, r.i);
-                R[((tr * (N - 3) + islot) * 2 + hi) * 6 + jslot * 2 + hj] = r;
+                if constexpr (kPacked<T>) {
+                    const unsigned row = (tr * (N - 3) + islot) * 2 + hi, w = 4u >> jslot;   // bit of h_j in h_T
+#pragma unroll
+                    for (unsigned ht = 0; ht < 8; ++ht)
+                        if (((ht / w) & 1u) == hj) R[row * kPackRow + pack_off(ht) + jslot] = r;
+                } else {
+                    R[((tr * (N - 3) + islot) * 2 + hi) * 6 + jslot * 2 + hj] = r;
+                }
             }
     }
     __syncthreads();
@@ -234,11 +269,17 @@ struct ChainBottom {
                 const int below = (p < idx[i]) + (q < idx[i]) + (r < idx[i]);
                 constexpr unsigned EB = sizeof(Cx<T>);
                 const int t = r * (r - 1) * (r - 2) / 6 + q * (q - 1) / 2 + p;
-                const unsigned R = rp[t] + io[idx[i]] - 12 * EB * below;
-                const Cx<T> r0 = lds_cx(R + hb[p], T()), r1 = lds_cx(R + hb[q] + 2 * EB, T()),
-                            r2 = lds_cx(R + hb[r] + 4 * EB, T());
-                Cx<T> k0, k1, k2;
-                lds_cx3(kt[t], k0, k1, k2);
+                Cx<T> r0, r1, r2, k0, k1, k2;
+                if constexpr (kPacked<T>) {
+                    lds_cx3_packed(rp[t] + io[idx[i]] - 2 * kPackRow * EB * below, r0, r1, r2);
+                    lds_cx3_packed(kt[t], k0, k1, k2);
+                } else {
+                    const unsigned R = rp[t] + io[idx[i]] - 12 * EB * below;
+                    r0 = lds_cx(R + hb[p], T());
+                    r1 = lds_cx(R + hb[q] + 2 * EB, T());
+                    r2 = lds_cx(R + hb[r] + 4 * EB, T());
+                    lds_cx3(kt[t], k0, k1, k2);
+                }
                 chain_acc(r0.r, r0.i, k0.r, k0.i, cr, ci);
                 chain_acc(r1.r, r1.i, k1.r, k1.i, cr, ci);
                 chain_acc(r2.r, r2.i, k2.r, k2.i, cr, ci);
@@ -298,7 +339,7 @@ struct WalkChain {
                 idx[m] = m;
                 photon[m] = i;
                 hb[m] = EB * hbit[m];
-                io[m] = EB * (12 * i + 6 * hbit[m]);
+                io[m] = kPacked<T> ? EB * kPackRow * (2 * i + hbit[m]) : EB * (12 * i + 6 * hbit[m]);
             }
             const unsigned k_base = (unsigned)__cvta_generic_to_shared(Kt), r_base = (unsigned)__cvta_generic_to_shared(Rt);
             unsigned rp[KT], kt[KT];
@@ -309,9 +350,16 @@ struct WalkChain {
 #pragma unroll
                     for (int p = 0; p < q; ++p) {  // colex rank of the photon triple
                         const int tr = photon[r] * (photon[r] - 1) * (photon[r] - 2) / 6 + photon[q] * (photon[q] - 1) / 2 + photon[p];
-                        rp[r * (r - 1) * (r - 2) / 6 + q * (q - 1) / 2 + p] = r_base + EB * (tr * (12 * (N - 3)));
-                        kt[r * (r - 1) * (r - 2) / 6 + q * (q - 1) / 2 + p] =
-                            k_base + EB * (tr * 24 + 4 * hbit[p] + 2 * hbit[q] + hbit[r]);
+                        const int t = r * (r - 1) * (r - 2) / 6 + q * (q - 1) / 2 + p;
+                        if constexpr (kPacked<T>) {
+                            // chunk of this lane's h_T = 4 h_p + 2 h_q + h_r: pack_off is additive in the three bits
+                            const unsigned hoff = EB * (pack_off(4) * hbit[p] + pack_off(2) * hbit[q] + pack_off(1) * hbit[r]);
+                            rp[t] = r_base + EB * (tr * (2 * kPackRow * (N - 3))) + hoff;
+                            kt[t] = k_base + EB * (tr * kPackRow) + hoff;
+                        } else {
+                            rp[t] = r_base + EB * (tr * (12 * (N - 3)));
+                            kt[t] = k_base + EB * (tr * 24 + 4 * hbit[p] + 2 * hbit[q] + hbit[r]);
+                        }
                     }
             ChainBottom<KB, KB, T, EA>::run(P + used, bit, e, idx, kt, rp, io, hb, v, ar, ai);
         } else {
